@@ -1,0 +1,165 @@
+/*
+ * gravidy_b200.h -- C-ABI boundary of the B200-native Hermite force/jerk hot path.
+ *
+ * The calls follow the paper's statement of the integration scheme (GraviDy, arXiv 1702.00440;
+ * "P:<n>" = line n of the paper text): steps (i)-(vii) of section 2.4.
+ *
+ *   gd_init                  steps (i)-(iv)  P:123-126   allocate/initialise, initial a and jerk (O(N^2)), initial dt
+ *   gd_next_block            step  (v)       P:127       find the particles to move at the next integration time
+ *   gd_predict               step  (vii-a)   P:130       predict x, v of ALL N particles to time t
+ *   gd_force_jerk            step  (vii-c)   P:132-136   a and jerk of the active particles from all N (Eq. 3, fn. 11 P:188)
+ *   gd_correct_and_timestep  steps (vi),(vii-d,e) P:128, P:137-138, P:241   corrector + Aarseth time-step update
+ *   gd_energy                Eq. 2           P:71, P:125 kinetic + (softened) potential energy
+ *
+ * Conventions
+ *   - All floating point is IEEE binary64.  Indices are int32.  G = 1 (N-body units).
+ *   - Pointers named *_dev are DEVICE pointers, *_host are HOST pointers.  The library never allocates
+ *     device memory: the caller hands one workspace of gd_workspace_bytes(n) bytes (256-byte aligned) to
+ *     gd_init and keeps it alive until gd_destroy.  Inputs are copied at init and may be freed afterwards.
+ *   - [n,3] arrays are row-major (x0 y0 z0 x1 y1 z1 ...).
+ *   - All work is enqueued on the CUDA stream given at init (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream).  Calls are asynchronous unless stated; the ones that return values to the
+ *     host (gd_next_block, gd_energy, gd_get_*_host, gd_*_host) synchronise that stream.
+ *   - Every call returns GD_OK (0) or a negative error code; the text of the last error is available from
+ *     gd_last_error().  After an error the only guaranteed-safe call is gd_destroy.
+ *   - Call order inside one block step: gd_next_block -> gd_predict(t_next) -> gd_force_jerk(NULL list)
+ *     -> gd_correct_and_timestep.  gd_step / gd_run_until replay exactly that sequence.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with GD_ECUDA.
+ */
+#ifndef GRAVIDY_B200_H
+#define GRAVIDY_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define GD_API __attribute__((visibility("default")))
+#else
+#define GD_API
+#endif
+
+#define GD_OK        0
+#define GD_EINVAL   -1   /* bad argument: n < 1, NaN or <= 0 eta, eps < 0, NULL pointer, workspace too small/misaligned */
+#define GD_ESTATE   -2   /* call order violated (e.g. correct before force) */
+#define GD_ECUDA    -3   /* CUDA runtime error (sticky); text via gd_last_error */
+
+/* Block-time-step limits (powers of two; the paper does not print them -- DESIGN.md reading R6). */
+#define GD_LEVEL_MIN 3    /* dt_max = 2^-3  */
+#define GD_LEVEL_MAX 23   /* dt_min = 2^-23 */
+
+typedef struct gd_ctx gd_ctx;   /* opaque; created by gd_init, destroyed by gd_destroy */
+
+/* Library / build identification: "gravidy_b200 <version> sm_100a". Never fails. */
+GD_API const char *gd_version(void);
+
+/* Bytes of device memory gd_init needs for n particles (state, predicted records, active list, force
+ * outputs, partial sums, scan scratch).  Returns 0 for n < 1. */
+GD_API size_t gd_workspace_bytes(int64_t n);
+
+/* Steps (i)-(iv).  Copies m [n], x [n,3], v [n,3] (device pointers) into the workspace, sets
+ * t = 0 and t_i = 0, evaluates a_i and jerk_i of every particle from the unpredicted state (one all-active
+ * gd_force_jerk, O(N^2)), and sets the initial block step dt_i = largest 2^-k <= eta |a_i| / |jerk_i|,
+ * clamped to [2^-GD_LEVEL_MAX, 2^-GD_LEVEL_MIN] (|jerk| = 0 -> dt_max).  eps is the softening length
+ * (>= 0; Eq. 3), eta the accuracy parameter of the time-step criterion (> 0).
+ * On success *out owns a small host struct; release it with gd_destroy.  Asynchronous. */
+GD_API int gd_init(gd_ctx **out, int64_t n, const double *m_dev, const double *x_dev, const double *v_dev,
+            double eps, double eta, void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Same as gd_init with HOST input arrays (pageable or pinned): the host->device copies are part of the
+ * call.  Used for end-to-end timing. */
+GD_API int gd_init_host(gd_ctx **out, int64_t n, const double *m_host, const double *x_host, const double *v_host,
+                 double eps, double eta, void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Releases the host struct (not the workspace).  NULL is allowed. */
+GD_API void gd_destroy(gd_ctx *ctx);
+
+/* Text of the last error recorded on ctx (ctx == NULL: last error of a failed gd_init). Never NULL. */
+GD_API const char *gd_last_error(const gd_ctx *ctx);
+
+/* Tunables.  key: "jsplit_max_nact" (active sets of at most this size use the j-split kernel; default 2048),
+ * "dt_level_min", "dt_level_max" (override GD_LEVEL_MIN/MAX before the first step; 0 <= min <= max <= 52),
+ * "halving_mode" (0: one halving per step [default]; 1: halve until dt <= dt_req).  GD_EINVAL on unknown keys. */
+GD_API int gd_set_option(gd_ctx *ctx, const char *key, double value);
+
+/* Step (v).  t_next = min_i (t_i + dt_i); the active list becomes { i ascending : t_i + dt_i == t_next }
+ * (exact comparison of dyadic doubles).  Writes t_next and the active count to the host pointers (either may
+ * be NULL).  Synchronises the stream. */
+GD_API int gd_next_block(gd_ctx *ctx, double *t_next_host, int64_t *n_act_host);
+
+/* Step (vii-a).  For ALL n particles, D = t - t_i:
+ *   xp = x + v D + a D^2/2 + jerk D^3/6 ;  vp = v + a D + jerk D^2/2
+ * written to the packed predicted records the force kernels read.  Sets the context's current time to t. */
+GD_API int gd_predict(gd_ctx *ctx, double t);
+
+/* Step (vii-c); Eq. 3 P:145 and its time derivative (sign per fn. 11 P:188).  For each listed i:
+ *   a_i    = sum_{j != i} m_j r_ij / (r_ij^2 + eps^2)^(3/2)
+ *   jerk_i = sum_{j != i} m_j [ v_ij / (r_ij^2 + eps^2)^(3/2) - 3 (r_ij . v_ij) r_ij / (r_ij^2 + eps^2)^(5/2) ]
+ * with r_ij = xp_j - xp_i, v_ij = vp_j - vp_i over the predicted records of all n particles (a prior gd_predict
+ * is required).  idx_dev: n_act int32 particle indices in [0, n) (device), or NULL for the internal active list
+ * of the last gd_next_block (then n_act is ignored).  a_out_dev / j_out_dev: [n_act,3] device arrays, or NULL
+ * to keep the results in the internal buffers that gd_correct_and_timestep consumes.  With an explicit
+ * idx_dev the call does not touch integrator state.  Indices are not range-checked.  n_act == 0 is a no-op.
+ * Large lists use the i-parallel kernel, small lists the j-split kernel (see "jsplit_max_nact"). */
+GD_API int gd_force_jerk(gd_ctx *ctx, const int32_t *idx_dev, int64_t n_act, double *a_out_dev, double *j_out_dev);
+
+/* One-shot form of gd_force_jerk on HOST arrays: x, v are taken as the (already predicted) state of n sources,
+ * idx_host (or NULL = all n) lists the sinks, results go to host arrays [n_act,3].  All copies are inside the call. */
+GD_API int gd_force_jerk_host(int64_t n, const double *m_host, const double *x_host, const double *v_host, double eps,
+                       const int32_t *idx_host, int64_t n_act, double *a_out_host, double *j_out_host,
+                       void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Steps (vi), (vii-d), (vii-e).  For every particle of the internal active list, with
+ * h = dt_i, (a0, j0) the stored values and (a1, j1) the results of the last gd_force_jerk(NULL list):
+ *   a2 = (-6 (a0 - a1) - h (4 j0 + 2 j1)) / h^2 ;  a3 = (12 (a0 - a1) + 6 h (j0 + j1)) / h^3
+ *   x = xp + a2 h^4/24 + a3 h^5/120 ;  v = vp + a2 h^3/6 + a3 h^4/24 ;  a2e = a2 + h a3
+ *   dt_req = sqrt( eta (|a1||a2e| + |j1|^2) / (|j1||a3| + |a2e|^2) )          (denominator 0 -> +inf)
+ *   dt_i <- h/2 if dt_req < h ; 2h if dt_req >= 2h and t_next is a multiple of 2h ; else h ; clamped
+ *   a_i <- a1, jerk_i <- j1, t_i <- t_next.
+ * GD_ESTATE unless preceded by next_block, predict(t_next) and force_jerk(NULL). */
+GD_API int gd_correct_and_timestep(gd_ctx *ctx);
+
+/* Eq. 2, P:71 (potential softened consistently with Eq. 3 -- DESIGN.md reading R8):
+ *   K = 1/2 sum m_i |v_i|^2 ;  U = - sum_{i<j} m_i m_j / sqrt(|r_ij|^2 + eps^2)
+ * evaluated on all particles predicted to the current time (identical to the stored state when every particle
+ * is synchronised).  Overwrites the predicted records.  Synchronises. */
+GD_API int gd_energy(gd_ctx *ctx, double *kinetic_host, double *potential_host);
+
+/* Convenience: n_steps block steps (next_block, predict, force_jerk, correct) / block steps until t >= t_end.
+ * Optional outputs (NULL to skip): steps taken, sum of active counts (particle steps).  Synchronises. */
+GD_API int gd_step(gd_ctx *ctx, int64_t n_steps, int64_t *particle_steps_host);
+GD_API int gd_run_until(gd_ctx *ctx, double t_end, int64_t max_steps, int64_t *steps_host, int64_t *particle_steps_host);
+
+/* Current time / counters.  Never fail on a valid ctx. */
+GD_API double  gd_time(const gd_ctx *ctx);
+GD_API int64_t gd_n(const gd_ctx *ctx);
+GD_API int64_t gd_n_active(const gd_ctx *ctx);          /* size of the current internal active list */
+GD_API int64_t gd_block_steps(const gd_ctx *ctx);       /* "Iter"   of Listing 1 */
+GD_API int64_t gd_particle_steps(const gd_ctx *ctx);    /* "Nsteps" of Listing 1 */
+GD_API int     gd_last_force_kernel(const gd_ctx *ctx); /* 0 none, 1 i-parallel, 2 j-split */
+GD_API int64_t gd_kernel_launches(const gd_ctx *ctx);   /* kernels launched on behalf of this ctx so far */
+
+/* Copies of the state into DEVICE arrays ([n,3] or [n]); any pointer may be NULL.  Asynchronous. */
+GD_API int gd_get_state(gd_ctx *ctx, double *x_dev, double *v_dev, double *a_dev, double *j_dev, double *t_dev, double *dt_dev);
+/* Same into HOST arrays; synchronises. */
+GD_API int gd_get_state_host(gd_ctx *ctx, double *x_host, double *v_host, double *a_host, double *j_host, double *t_host, double *dt_host);
+/* Predicted positions / velocities of the last gd_predict into DEVICE arrays [n,3]. */
+GD_API int gd_get_predicted(gd_ctx *ctx, double *xp_dev, double *vp_dev);
+/* Current internal active list into a device array of capacity cap (>= gd_n_active). */
+GD_API int gd_get_active(gd_ctx *ctx, int32_t *idx_dev, int64_t cap);
+/* Particle steps taken per level k (dt = 2^-k) since init -> counts_host[64]; and diagnostic counters
+ * diag_host[2] = { time-step criteria that evaluated to NaN, clamps at dt_min }.  Synchronises. */
+GD_API int gd_get_level_histogram(gd_ctx *ctx, int64_t *counts_host, int64_t *diag_host);
+
+/* Register-only DFMA loop on every SM: measures the FP64 peak the force kernels are bounded by.  Returns the
+ * achieved rate in flop/s (2 flop per FMA per lane) in *flops_host; ms_host receives the elapsed milliseconds.
+ * Needs no ctx (it allocates and frees 8 bytes of device memory itself).  Synchronises the device. */
+GD_API int gd_fp64_peak_probe(int iters, double *flops_host, double *ms_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRAVIDY_B200_H */

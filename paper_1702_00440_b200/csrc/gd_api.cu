@@ -1,0 +1,423 @@
+// gd_api.cu -- the C-ABI of include/gravidy_b200.h: argument checks, workspace carving, call-order state and
+// the sequencing of the kernels.  No arithmetic of the method lives here.
+#include "gd_common.cuh"
+#include "../../include/gravidy_b200.h"
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+static char g_init_err[512] = "";
+
+int gd_fail_cuda(gd_ctx *c, cudaError_t e, const char *what)
+{
+    char *dst = c ? c->err : g_init_err;
+    snprintf(dst, 512, "CUDA error %d (%s) at %s", (int)e, cudaGetErrorString(e), what);
+    return GD_ECUDA;
+}
+
+static int gd_fail(gd_ctx *c, int code, const char *msg)
+{
+    char *dst = c ? c->err : g_init_err;
+    snprintf(dst, 512, "%s", msg);
+    return code;
+}
+
+// ---- workspace -------------------------------------------------------------------------------------------
+static inline int64_t gd_pad(int64_t n) { return ((n + GD_TILE_J - 1) / GD_TILE_J) * GD_TILE_J; }
+static inline int64_t gd_pcap(int64_t np) { return (4 * np > (1 << 20)) ? 4 * np : (1 << 20); }
+static inline size_t gd_up(size_t b) { return (b + 255) & ~(size_t)255; }
+
+struct gd_carver {
+    char *base;
+    size_t off;
+    template <typename T> T *take(size_t count)
+    {
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += gd_up(count * sizeof(T));
+        return p;
+    }
+};
+
+static size_t gd_carve(gd_dev *d, void *base, int64_t np, int64_t pcap)
+{
+    gd_carver w{(char *)base, 0};
+    gd_dev t;
+    t.xm = w.take<double4>(np);
+    t.vt = w.take<double4>(np);
+    t.ad = w.take<double4>(np);
+    t.jk = w.take<double4>(np);
+    t.tnext = w.take<double>(np);
+    t.pxy = w.take<double2>(np);
+    t.pzm = w.take<double2>(np);
+    t.vxy = w.take<double2>(np);
+    t.vz = w.take<double>(np);
+    t.idx = w.take<int32_t>(np);
+    t.a1 = w.take<double>(3 * np);
+    t.j1 = w.take<double>(3 * np);
+    t.partial = w.take<double>(6 * pcap);
+    t.blockmin = w.take<double>(GD_SCAN_MAX_BLOCKS);
+    t.agg = w.take<unsigned long long>(GD_SCAN_MAX_BLOCKS);
+    t.ticket = w.take<unsigned int>(4);
+    t.cell = w.take<double>(4);
+    t.hist = w.take<long long>(64);
+    t.diag = w.take<long long>(2);
+    t.phi = w.take<double>(np);
+    t.kin = w.take<double>(np);
+    t.staging = w.take<double>(7 * np);
+    if (d) *d = t;
+    return w.off;
+}
+
+extern "C" const char *gd_version(void) { return "gravidy_b200 0.1 sm_100a"; }
+
+extern "C" size_t gd_workspace_bytes(int64_t n)
+{
+    if (n < 1) return 0;
+    int64_t np = gd_pad(n);
+    return gd_carve(nullptr, nullptr, np, gd_pcap(np));
+}
+
+extern "C" const char *gd_last_error(const gd_ctx *ctx) { return ctx ? ctx->err : g_init_err; }
+
+extern "C" void gd_destroy(gd_ctx *ctx)
+{
+    if (!ctx) return;
+    if (ctx->h_cell) cudaFreeHost(ctx->h_cell);
+    free(ctx);
+}
+
+// ---- init ------------------------------------------------------------------------------------------------
+static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, size_t ws_bytes, void *stream)
+{
+    if (!out) return gd_fail(nullptr, GD_EINVAL, "gd_init: out is NULL");
+    *out = nullptr;
+    if (n < 1 || n > (int64_t)1 << 30) return gd_fail(nullptr, GD_EINVAL, "gd_init: n out of range");
+    if (!(eta > 0.0) || !(eps >= 0.0) || !isfinite(eta) || !isfinite(eps)) return gd_fail(nullptr, GD_EINVAL, "gd_init: need eta > 0 and eps >= 0");
+    if (!ws || ((uintptr_t)ws & 255)) return gd_fail(nullptr, GD_EINVAL, "gd_init: workspace NULL or not 256-byte aligned");
+    if (ws_bytes < gd_workspace_bytes(n)) return gd_fail(nullptr, GD_EINVAL, "gd_init: workspace too small (see gd_workspace_bytes)");
+    gd_ctx *c = (gd_ctx *)calloc(1, sizeof(gd_ctx));
+    if (!c) return gd_fail(nullptr, GD_EINVAL, "gd_init: out of host memory");
+    c->n = n;
+    c->np = gd_pad(n);
+    c->pcap = gd_pcap(c->np);
+    c->eps = eps;
+    c->eps2 = eps * eps;
+    c->eta = eta;
+    c->lvl_min = GD_LEVEL_MIN;
+    c->lvl_max = GD_LEVEL_MAX;
+    c->dt_max = ldexp(1.0, -GD_LEVEL_MIN);
+    c->dt_min = ldexp(1.0, -GD_LEVEL_MAX);
+    c->halving_mode = 0;
+    c->jsplit_max_nact = 2048;
+    c->stream = (cudaStream_t)stream;
+    gd_carve(&c->d, ws, c->np, c->pcap);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaHostAlloc((void **)&c->h_cell, 64, cudaHostAllocDefault);
+    if (e != cudaSuccess) {
+        gd_fail_cuda(nullptr, e, "gd_init: no usable CUDA device (there is no CPU fallback)");
+        free(c);
+        return GD_ECUDA;
+    }
+    *out = c;
+    return GD_OK;
+}
+
+static int gd_init_common(gd_ctx *c, const double *m_dev, const double *x_dev, const double *v_dev)
+{
+    // scan scratch, histogram, diagnostics start from zero (epoch 0 = "never written")
+    GD_CUDA(c, cudaMemsetAsync(c->d.blockmin, 0, (char *)c->d.phi - (char *)c->d.blockmin, c->stream));
+    c->epoch = 0;
+    c->ticket_min_base = c->ticket_cmp_base = 0;
+    int rc;
+    if ((rc = gdk_pack_state(c, m_dev, x_dev, v_dev))) return rc;          // also the predicted records at t = 0
+    c->t = 0.0;
+    c->t_pred = 0.0;
+    c->have_pred = true;
+    // steps (iii)-(iv): initial a, jerk of every particle from the unpredicted state, then the initial dt
+    if ((rc = gdk_force(c, nullptr, c->n, c->d.a1, c->d.j1))) return rc;
+    if ((rc = gdk_initial_dt(c))) return rc;
+    c->have_block = c->have_force = false;
+    c->n_act = 0;
+    return GD_OK;
+}
+
+extern "C" int gd_init(gd_ctx **out, int64_t n, const double *m_dev, const double *x_dev, const double *v_dev, double eps,
+                       double eta, void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!m_dev || !x_dev || !v_dev) return gd_fail(nullptr, GD_EINVAL, "gd_init: NULL input array");
+    int rc = gd_create(out, n, eps, eta, workspace_dev, workspace_bytes, cuda_stream);
+    if (rc) return rc;
+    rc = gd_init_common(*out, m_dev, x_dev, v_dev);
+    if (rc) { snprintf(g_init_err, sizeof g_init_err, "%s", (*out)->err); gd_destroy(*out); *out = nullptr; }
+    return rc;
+}
+
+extern "C" int gd_init_host(gd_ctx **out, int64_t n, const double *m_host, const double *x_host, const double *v_host,
+                            double eps, double eta, void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!m_host || !x_host || !v_host) return gd_fail(nullptr, GD_EINVAL, "gd_init_host: NULL input array");
+    int rc = gd_create(out, n, eps, eta, workspace_dev, workspace_bytes, cuda_stream);
+    if (rc) return rc;
+    gd_ctx *c = *out;
+    double *st = (double *)c->d.staging;
+    cudaError_t e = cudaMemcpyAsync(st, m_host, n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(st + c->np, x_host, 3 * n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(st + 4 * c->np, v_host, 3 * n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    rc = (e == cudaSuccess) ? gd_init_common(c, st, st + c->np, st + 4 * c->np) : gd_fail_cuda(c, e, "gd_init_host: H2D copy");
+    if (rc) { snprintf(g_init_err, sizeof g_init_err, "%s", c->err); gd_destroy(c); *out = nullptr; }
+    return rc;
+}
+
+extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
+{
+    if (!c || !key) return GD_EINVAL;
+    if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; return GD_OK; }
+    if (!strcmp(key, "halving_mode")) { c->halving_mode = value != 0.0; return GD_OK; }
+    if (!strcmp(key, "dt_level_min") || !strcmp(key, "dt_level_max")) {
+        int lv = (int)value;
+        if (lv < 0 || lv > 52) return gd_fail(c, GD_EINVAL, "gd_set_option: level out of range");
+        if (c->block_steps > 0) return gd_fail(c, GD_ESTATE, "gd_set_option: levels can only change before the first step");
+        int lo = !strcmp(key, "dt_level_min") ? lv : c->lvl_min, hi = !strcmp(key, "dt_level_max") ? lv : c->lvl_max;
+        c->lvl_min = lo;
+        c->lvl_max = hi;
+        if (lo > hi) return GD_OK;                 // transient while the caller sets both; checked below once ordered
+        c->dt_max = ldexp(1.0, -lo);
+        c->dt_min = ldexp(1.0, -hi);
+        // the initial steps depend on the limits: redo them from the stored a, jerk
+        int rc = gdk_unpack_state(c, nullptr, nullptr, c->d.a1, c->d.j1, nullptr, nullptr);
+        if (!rc) rc = gdk_initial_dt(c);
+        return rc;
+    }
+    return gd_fail(c, GD_EINVAL, "gd_set_option: unknown key");
+}
+
+// ---- the five stages ----------------------------------------------------------------------------------------
+extern "C" int gd_next_block(gd_ctx *c, double *t_next_host, int64_t *n_act_host)
+{
+    if (!c) return GD_EINVAL;
+    if (c->lvl_min > c->lvl_max) return gd_fail(c, GD_ESTATE, "gd_next_block: dt_level_min > dt_level_max");
+    int rc = gdk_next_block(c);
+    if (rc) return rc == GD_ECUDA ? rc : GD_EINVAL;          // text already in c->err
+    GD_CUDA(c, cudaMemcpyAsync(c->h_cell, c->d.cell, 16, cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->t_next = c->h_cell[0];
+    long long na;
+    memcpy(&na, &c->h_cell[1], 8);
+    c->n_act = na;
+    c->have_block = true;
+    c->have_force = false;
+    if (t_next_host) *t_next_host = c->t_next;
+    if (n_act_host) *n_act_host = c->n_act;
+    return GD_OK;
+}
+
+extern "C" int gd_predict(gd_ctx *c, double t)
+{
+    if (!c) return GD_EINVAL;
+    if (t != t) return gd_fail(c, GD_EINVAL, "gd_predict: t is NaN");
+    int rc = gdk_predict(c, t);
+    if (rc) return rc;
+    c->t_pred = t;
+    c->have_pred = true;
+    c->have_force = false;
+    return GD_OK;
+}
+
+extern "C" int gd_force_jerk(gd_ctx *c, const int32_t *idx_dev, int64_t n_act, double *a_out_dev, double *j_out_dev)
+{
+    if (!c) return GD_EINVAL;
+    if (!c->have_pred) return gd_fail(c, GD_ESTATE, "gd_force_jerk: no predicted records (call gd_predict first)");
+    if ((a_out_dev == nullptr) != (j_out_dev == nullptr)) return gd_fail(c, GD_EINVAL, "gd_force_jerk: give both outputs or neither");
+    if (!idx_dev) {
+        if (!c->have_block) return gd_fail(c, GD_ESTATE, "gd_force_jerk: no internal active list (call gd_next_block first)");
+        int rc = gdk_force(c, c->d.idx, c->n_act, a_out_dev ? a_out_dev : c->d.a1, j_out_dev ? j_out_dev : c->d.j1);
+        if (rc) return rc;
+        if (!a_out_dev) c->have_force = (c->t_pred == c->t_next);
+        return GD_OK;
+    }
+    if (n_act < 0 || n_act > c->np) return gd_fail(c, GD_EINVAL, "gd_force_jerk: n_act out of range");
+    if (!a_out_dev) return gd_fail(c, GD_EINVAL, "gd_force_jerk: explicit index list needs explicit outputs");
+    return gdk_force(c, idx_dev, n_act, a_out_dev, j_out_dev);
+}
+
+extern "C" int gd_correct_and_timestep(gd_ctx *c)
+{
+    if (!c) return GD_EINVAL;
+    if (!c->have_block || !c->have_force)
+        return gd_fail(c, GD_ESTATE, "gd_correct_and_timestep: needs gd_next_block, gd_predict(t_next), gd_force_jerk(NULL) first");
+    int rc = gdk_correct(c, c->t_next);
+    if (rc) return rc;
+    c->t = c->t_next;
+    c->block_steps += 1;
+    c->particle_steps += c->n_act;
+    c->have_block = c->have_force = false;
+    c->have_pred = false;                  // the predicted records of the corrected particles are stale now
+    return GD_OK;
+}
+
+extern "C" int gd_energy(gd_ctx *c, double *kinetic_host, double *potential_host)
+{
+    if (!c) return GD_EINVAL;
+    int rc = gdk_predict(c, c->t);
+    if (rc) return rc;
+    c->t_pred = c->t;
+    c->have_pred = true;
+    c->have_force = false;
+    if ((rc = gdk_energy(c))) return rc;
+    GD_CUDA(c, cudaMemcpyAsync(c->h_cell + 2, c->d.cell + 2, 16, cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (kinetic_host) *kinetic_host = c->h_cell[2];
+    if (potential_host) *potential_host = c->h_cell[3];
+    return GD_OK;
+}
+
+static int gd_one_step(gd_ctx *c)
+{
+    int rc = gd_next_block(c, nullptr, nullptr);
+    if (!rc) rc = gd_predict(c, c->t_next);
+    if (!rc) rc = gd_force_jerk(c, nullptr, 0, nullptr, nullptr);
+    if (!rc) rc = gd_correct_and_timestep(c);
+    return rc;
+}
+
+extern "C" int gd_step(gd_ctx *c, int64_t n_steps, int64_t *particle_steps_host)
+{
+    if (!c) return GD_EINVAL;
+    int64_t before = c->particle_steps;
+    for (int64_t s = 0; s < n_steps; ++s) {
+        int rc = gd_one_step(c);
+        if (rc) return rc;
+    }
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (particle_steps_host) *particle_steps_host = c->particle_steps - before;
+    return GD_OK;
+}
+
+extern "C" int gd_run_until(gd_ctx *c, double t_end, int64_t max_steps, int64_t *steps_host, int64_t *particle_steps_host)
+{
+    if (!c) return GD_EINVAL;
+    int64_t before = c->particle_steps, steps = 0;
+    while (c->t < t_end && (max_steps < 0 || steps < max_steps)) {
+        int rc = gd_one_step(c);
+        if (rc) return rc;
+        ++steps;
+    }
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (steps_host) *steps_host = steps;
+    if (particle_steps_host) *particle_steps_host = c->particle_steps - before;
+    return GD_OK;
+}
+
+// ---- getters -----------------------------------------------------------------------------------------------
+extern "C" double gd_time(const gd_ctx *c) { return c ? c->t : NAN; }
+extern "C" int64_t gd_n(const gd_ctx *c) { return c ? c->n : 0; }
+extern "C" int64_t gd_n_active(const gd_ctx *c) { return c && c->have_block ? c->n_act : 0; }
+extern "C" int64_t gd_block_steps(const gd_ctx *c) { return c ? c->block_steps : 0; }
+extern "C" int64_t gd_particle_steps(const gd_ctx *c) { return c ? c->particle_steps : 0; }
+extern "C" int gd_last_force_kernel(const gd_ctx *c) { return c ? c->last_force_kernel : 0; }
+extern "C" int64_t gd_kernel_launches(const gd_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" int gd_get_state(gd_ctx *c, double *x, double *v, double *a, double *j, double *t, double *dt)
+{
+    if (!c) return GD_EINVAL;
+    return gdk_unpack_state(c, x, v, a, j, t, dt);
+}
+
+extern "C" int gd_get_state_host(gd_ctx *c, double *x, double *v, double *a, double *j, double *t, double *dt)
+{
+    if (!c) return GD_EINVAL;
+    // unpack into the staging area ([np,3] x 4 would not fit: two passes of at most 7 np doubles)
+    double *st = (double *)c->d.staging;
+    const int64_t n = c->n, np = c->np;
+    if (x || v) {
+        int rc = gdk_unpack_state(c, x ? st : nullptr, v ? st + 3 * np : nullptr, nullptr, nullptr, nullptr, nullptr);
+        if (rc) return rc;
+        if (x) GD_CUDA(c, cudaMemcpyAsync(x, st, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        if (v) GD_CUDA(c, cudaMemcpyAsync(v, st + 3 * np, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    }
+    if (a || j || t || dt) {
+        if (x || v) GD_CUDA(c, cudaStreamSynchronize(c->stream));
+        int rc = gdk_unpack_state(c, nullptr, nullptr, a ? st : nullptr, j ? st + 3 * np : nullptr, t ? st + 6 * np : nullptr, nullptr);
+        if (rc) return rc;
+        if (a) GD_CUDA(c, cudaMemcpyAsync(a, st, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        if (j) GD_CUDA(c, cudaMemcpyAsync(j, st + 3 * np, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        if (t) GD_CUDA(c, cudaMemcpyAsync(t, st + 6 * np, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        if (dt) {
+            GD_CUDA(c, cudaStreamSynchronize(c->stream));
+            rc = gdk_unpack_state(c, nullptr, nullptr, nullptr, nullptr, nullptr, st);
+            if (rc) return rc;
+            GD_CUDA(c, cudaMemcpyAsync(dt, st, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        }
+    }
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return GD_OK;
+}
+
+extern "C" int gd_get_predicted(gd_ctx *c, double *xp, double *vp)
+{
+    if (!c) return GD_EINVAL;
+    if (!c->have_pred) return gd_fail(c, GD_ESTATE, "gd_get_predicted: no predicted records");
+    return gdk_unpack_predicted(c, xp, vp);
+}
+
+extern "C" int gd_get_active(gd_ctx *c, int32_t *idx_dev, int64_t cap)
+{
+    if (!c || !idx_dev) return GD_EINVAL;
+    if (!c->have_block) return gd_fail(c, GD_ESTATE, "gd_get_active: no active list");
+    if (cap < c->n_act) return gd_fail(c, GD_EINVAL, "gd_get_active: capacity too small");
+    if (c->n_act > 0)
+        GD_CUDA(c, cudaMemcpyAsync(idx_dev, c->d.idx, c->n_act * sizeof(int32_t), cudaMemcpyDeviceToDevice, c->stream));
+    return GD_OK;
+}
+
+extern "C" int gd_get_level_histogram(gd_ctx *c, int64_t *counts_host, int64_t *diag_host)
+{
+    if (!c) return GD_EINVAL;
+    if (counts_host) GD_CUDA(c, cudaMemcpyAsync(counts_host, c->d.hist, 64 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    if (diag_host) GD_CUDA(c, cudaMemcpyAsync(diag_host, c->d.diag, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return GD_OK;
+}
+
+// ---- one-shot host entry -------------------------------------------------------------------------------------
+extern "C" int gd_force_jerk_host(int64_t n, const double *m_host, const double *x_host, const double *v_host, double eps,
+                                  const int32_t *idx_host, int64_t n_act, double *a_out_host, double *j_out_host,
+                                  void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!m_host || !x_host || !v_host || !a_out_host || !j_out_host) return gd_fail(nullptr, GD_EINVAL, "gd_force_jerk_host: NULL array");
+    gd_ctx *c = nullptr;
+    int rc = gd_create(&c, n, eps, 1.0, workspace_dev, workspace_bytes, cuda_stream);
+    if (rc) return rc;
+    if (!idx_host) n_act = n;
+    if (n_act < 0 || n_act > n) { gd_destroy(c); return gd_fail(nullptr, GD_EINVAL, "gd_force_jerk_host: n_act out of range"); }
+    double *st = (double *)c->d.staging;
+    cudaError_t e = cudaMemcpyAsync(st, m_host, n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(st + c->np, x_host, 3 * n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(st + 4 * c->np, v_host, 3 * n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess && idx_host && n_act > 0)
+        e = cudaMemcpyAsync(c->d.idx, idx_host, n_act * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream);
+    if (e != cudaSuccess) rc = gd_fail_cuda(c, e, "gd_force_jerk_host: H2D copy");
+    if (!rc) rc = gdk_pack_sources(c, st, st + c->np, st + 4 * c->np);
+    if (!rc) rc = gdk_force(c, idx_host ? c->d.idx : nullptr, n_act, c->d.a1, c->d.j1);
+    if (!rc && n_act > 0) {
+        e = cudaMemcpyAsync(a_out_host, c->d.a1, 3 * n_act * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(j_out_host, c->d.j1, 3 * n_act * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+        if (e != cudaSuccess) rc = gd_fail_cuda(c, e, "gd_force_jerk_host: D2H copy");
+    }
+    if (!rc) {
+        e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) rc = gd_fail_cuda(c, e, "gd_force_jerk_host: synchronize");
+    }
+    if (rc) snprintf(g_init_err, sizeof g_init_err, "%s", c->err);
+    gd_destroy(c);
+    return rc;
+}
+
+extern "C" int gd_fp64_peak_probe(int iters, double *flops_host, double *ms_host)
+{
+    if (iters < 1) return GD_EINVAL;
+    return gdk_fp64_probe(iters, flops_host, ms_host) ? GD_ECUDA : GD_OK;
+}

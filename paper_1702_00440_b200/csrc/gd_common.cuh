@@ -1,0 +1,96 @@
+// gd_common.cuh -- shared declarations of the CUDA path (sm_100a only).  Not shared with oracle/.
+//
+// Device-resident state (all in the caller's workspace, every array 256-byte aligned; np = n rounded up to
+// GD_TILE_J, records n..np-1 are zero-mass padding):
+//   xm[np]  double4 {x, y, z, m}          vt[np] double4 {vx, vy, vz, t_i}
+//   ad[np]  double4 {ax, ay, az, dt_i}    jk[np] double4 {jx, jy, jz, 0}
+//   tnext[np] double  t_i + dt_i (exact dyadic; +inf in the padding)
+// Predicted records written by the predictor and read by the force kernels, as four coalesced SoA planes:
+//   pxy[np] double2 {xp, yp}   pzm[np] double2 {zp, m}   vxy[np] double2 {vxp, vyp}   vz[np] double {vzp}
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#define GD_TILE_J 256            // sources per shared-memory tile of the i-parallel kernel; np is a multiple
+
+struct gd_dev {
+    double4 *xm, *vt, *ad, *jk;
+    double *tnext;
+    double2 *pxy, *pzm, *vxy;
+    double *vz;
+    int32_t *idx;                // active list (ascending)
+    double *a1, *j1;             // [np,3] force results of the internal active list
+    double *partial;             // [pcap,6] partial sums of split force evaluations
+    double *blockmin;            // [GD_SCAN_MAX_BLOCKS] per-block minima of tnext
+    unsigned long long *agg;     // [GD_SCAN_MAX_BLOCKS] {epoch:32 | count:32} per-block aggregates of the compaction
+    unsigned int *ticket;        // [4] monotonically increasing block tickets (never reset)
+    double *cell;                // [4] {t_next, n_act (as int64 bits), K, U}
+    long long *hist;             // [64] particle steps per level
+    long long *diag;             // [2]  NaN criteria, dt_min clamps
+    double *phi;                 // [np] per-particle potential sums  (energy)
+    double *kin;                 // [np] per-particle kinetic terms   (energy)
+    void *staging;               // [7 np] doubles: staging for host<->device copies of m, x, v
+};
+
+#define GD_SCAN_MAX_BLOCKS 1024
+#define GD_SCAN_THREADS 1024
+
+struct gd_ctx {
+    int64_t n, np, pcap;
+    double eps, eps2, eta;
+    int lvl_min, lvl_max, halving_mode;
+    double dt_min, dt_max;
+    int64_t jsplit_max_nact;
+    cudaStream_t stream;
+    gd_dev d;
+    double *h_cell;              // pinned host mirror of d.cell
+    // host-side step state
+    double t, t_next;
+    int64_t n_act;
+    bool have_block, have_pred, have_force;
+    double t_pred;
+    int64_t block_steps, particle_steps, launches;
+    int last_force_kernel;
+    unsigned int epoch, ticket_min_base, ticket_cmp_base;
+    int sm_count;
+    char err[512];
+};
+
+// ---- launch wrappers (one per kernel file); all enqueue on c->stream and bump c->launches -------------
+int gdk_pack_state(gd_ctx *c, const double *m, const double *x, const double *v);           // gd_predict.cu
+int gdk_predict(gd_ctx *c, double t);
+int gdk_initial_dt(gd_ctx *c);
+int gdk_unpack_state(gd_ctx *c, double *x, double *v, double *a, double *j, double *t, double *dt);
+int gdk_unpack_predicted(gd_ctx *c, double *xp, double *vp);
+int gdk_pack_sources(gd_ctx *c, const double *m, const double *x, const double *v);
+int gdk_iota(gd_ctx *c, int32_t *idx, int64_t n);
+
+int gdk_force(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out);   // gd_force.cu
+
+int gdk_correct(gd_ctx *c, double t_next);                                                   // gd_correct.cu
+int gdk_next_block(gd_ctx *c);                                                               // gd_next_block.cu
+int gdk_energy(gd_ctx *c);                                                                   // gd_energy.cu
+int gdk_fp64_probe(int iters, double *flops, double *ms);                                    // gd_probe.cu
+
+int gd_fail_cuda(gd_ctx *c, cudaError_t e, const char *what);
+
+#define GD_CUDA(c, call)                                                     \
+    do {                                                                     \
+        cudaError_t e_ = (call);                                             \
+        if (e_ != cudaSuccess) return gd_fail_cuda((c), e_, #call);          \
+    } while (0)
+#define GD_LAUNCH_CHECK(c, name)                                             \
+    do {                                                                     \
+        cudaError_t e_ = cudaGetLastError();                                 \
+        if (e_ != cudaSuccess) return gd_fail_cuda((c), e_, name);           \
+        (c)->launches += 1;                                                  \
+    } while (0)
+
+// ---- small device helpers ---------------------------------------------------------------------------
+__device__ __forceinline__ double gd_norm3(double x, double y, double z)
+{
+    // sqrt((x*x + y*y) + z*z) with separately rounded operations (no contraction): the time-step decisions
+    // downstream are discrete, so the memory-bound kernels keep every rounding explicit.
+    return __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z)));
+}

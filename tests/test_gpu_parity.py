@@ -1,0 +1,286 @@
+"""Parity of the CUDA path (through the C-ABI, via the ctypes binding) with the CPU oracle, element by element
+on the same seeded inputs.  Tolerances:
+  * a, jerk: per-particle vector-norm relative error <= 1e-12 (north_star) against the oracle's compensated sums;
+  * predictor, corrector, time steps given identical inputs: bit-exact (both round every operation separately);
+  * active lists, block levels, times: bit-exact;
+  * energy: |dK/K|, |dU/U| <= 1e-13.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle
+from paper_1702_00440_b200 import workloads as W
+
+
+@pytest.fixture(scope="module")
+def gd():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (the product has no CPU fallback)")
+    from paper_1702_00440_b200 import binding
+    binding.load()
+    return binding
+
+
+def relnorm(u, ref):
+    u, ref = np.asarray(u, dtype=np.float64), np.asarray(ref, dtype=np.float64)
+    den = np.linalg.norm(ref, axis=-1)
+    den = np.where(den == 0, 1.0, den)
+    return np.linalg.norm(u - ref, axis=-1) / den
+
+
+def cpu(t):
+    return t.detach().cpu().numpy()
+
+
+TOL = 1e-12
+
+
+# ------------------------------------------------------------------------------------------- force / jerk
+@pytest.mark.parametrize("n", [1, 2, 3, 31, 257, 1000])
+@pytest.mark.parametrize("eps", [0.0, 1e-4])
+def test_force_small_and_ragged(gd, n, eps):
+    # tiny and ragged sizes: one tile with a tail, padding records, eps = 0 self-pair masking
+    w = W.random_cluster(n, seed=20 + n, eps=eps)
+    a, j = gd.force_jerk_host(w.m, w.x, w.v, eps)
+    a_ref, j_ref = oracle.pairsum(w.m, w.x, w.v, eps)
+    assert relnorm(a, a_ref).max() <= TOL and relnorm(j, j_ref).max() <= TOL
+    assert np.isfinite(a).all() and np.isfinite(j).all()
+
+
+def test_force_hand_example(gd):
+    # the paper-formula hand example of tests/golden/pairsum_hand_example.txt
+    from conftest import read_golden_table
+    m = np.array([0.0, 1.0])
+    x = np.array([[0, 0, 0], [3, 4, 0.0]])
+    v = np.array([[0, 0, 0], [1, 2, 0.0]])
+    for eps2, *ref in read_golden_table("pairsum_hand_example.txt"):
+        a, j = gd.force_jerk_host(m, x, v, math.sqrt(eps2))
+        assert np.allclose(a[0], ref[:3], rtol=1e-15, atol=1e-18) and np.allclose(j[0], ref[3:], rtol=2e-15, atol=1e-18)
+        assert not a[1].any() and not j[1].any()
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (2, 16384), (4, 5000), (5, 3000)])
+def test_force_all_active_configs(gd, cfg, n):
+    # all-active evaluation on the config inputs (C4: Kroupa masses; C5: central point mass, N = n + 1 ragged)
+    w = W.config(cfg, n=n)
+    a, j = gd.force_jerk_host(w.m, w.x, w.v, w.eps)
+    a_ref, j_ref = oracle.pairsum(w.m, w.x, w.v, w.eps)
+    ea, ej = relnorm(a, a_ref), relnorm(j, j_ref)
+    assert ea.max() <= TOL and ej.max() <= TOL, (ea.max(), ej.max())
+
+
+@pytest.mark.parametrize("kernel", ["ipar", "jsplit"])
+@pytest.mark.parametrize("n_act", [1, 5, 16, 100, 256, 1000, 4096])
+def test_force_active_subsets_both_kernels(gd, kernel, n_act):
+    # C3-style index sets on a smaller sphere, forced through each kernel; the two must agree with the oracle
+    import torch
+    w = W.config(3, n=8192 + 77)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h.set_option("jsplit_max_nact", 0 if kernel == "ipar" else 1 << 30)
+    h.predict(0.0)
+    idx = W.active_indices(w.n, n_act)
+    a, j = h.force_jerk(torch.from_numpy(idx).cuda())
+    assert h.last_force_kernel == kernel
+    a_ref, j_ref = oracle.pairsum(w.m, w.x, w.v, w.eps, idx=idx)
+    assert relnorm(cpu(a), a_ref).max() <= TOL and relnorm(cpu(j), j_ref).max() <= TOL
+    # run-to-run identical (fixed combination order)
+    a2, j2 = h.force_jerk(torch.from_numpy(idx).cuda())
+    assert torch.equal(a, a2) and torch.equal(j, j2)
+    h.close()
+
+
+def test_force_unsorted_and_repeated_indices(gd):
+    import torch
+    w = W.config(1)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h.predict(0.0)
+    idx = np.array([1023, 0, 5, 5, 512, 0], dtype=np.int32)
+    a, j = h.force_jerk(torch.from_numpy(idx).cuda())
+    a_ref, j_ref = oracle.pairsum(w.m, w.x, w.v, w.eps, idx=idx)
+    assert relnorm(cpu(a), a_ref).max() <= TOL and relnorm(cpu(j), j_ref).max() <= TOL
+    h.close()
+
+
+# ------------------------------------------------------------------------------ init, predictor, corrector
+def test_init_matches_oracle(gd):
+    w = W.config(1)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    s = {k: cpu(v) for k, v in h.state().items()}
+    assert np.array_equal(s["x"], w.x) and np.array_equal(s["v"], w.v)
+    assert relnorm(s["a"], o.a).max() <= TOL and relnorm(s["j"], o.j).max() <= TOL
+    assert np.array_equal(s["dt"], o.dt) and not s["t"].any()
+    h.close()
+
+
+def test_predictor_bit_exact_given_same_state(gd):
+    # advance the GPU a few steps, then predict both from the GPU's own state: identical inputs -> identical bits
+    w = W.config(1, n=700)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h.step(25)
+    s = {k: cpu(v) for k, v in h.state().items()}
+    t = h.t + 2.0 ** -9
+    h.predict(t)
+    xp, vp = (cpu(u) for u in h.predicted())
+    xp_ref, vp_ref = oracle.predict(t, s["x"], s["v"], s["a"], s["j"], s["t"])
+    assert np.array_equal(xp, xp_ref) and np.array_equal(vp, vp_ref)
+    h.close()
+
+
+def test_corrector_bit_exact_given_same_inputs(gd):
+    import torch
+    w = W.config(4, n=900)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h.step(10)
+    before = {k: cpu(v) for k, v in h.state().items()}
+    t_next, n_act = h.next_block()
+    act = cpu(h.active())
+    h.predict(t_next)
+    xp, vp = (cpu(u) for u in h.predicted())
+    a1 = torch.empty((n_act, 3), dtype=torch.float64, device="cuda")
+    j1 = torch.empty_like(a1)
+    h.force_jerk(None, a1, j1)            # explicit outputs: a copy of what the corrector will consume
+    h.force_jerk(None)
+    h.correct_and_timestep()
+    after = {k: cpu(v) for k, v in h.state().items()}
+    ref = oracle.correct(act, t_next, w.eta, before["x"], before["v"], before["a"], before["j"], before["t"],
+                         before["dt"], xp, vp, cpu(a1), cpu(j1))
+    for k, r in zip(("x", "v", "a", "j", "t", "dt"), ref):
+        assert np.array_equal(after[k], r), k
+    h.close()
+
+
+# ----------------------------------------------------------------------------------------- active sets
+def test_next_block_against_oracle_on_synthetic_times(gd):
+    # drive the compaction with many different patterns by stepping a small system; every list must be the
+    # ascending exact-equality set of the oracle's definition applied to the GPU's own t, dt
+    w = W.config(1, n=3000)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    for _ in range(30):
+        s = h.state(("t", "dt"))
+        t_ref, act_ref = oracle.next_block(cpu(s["t"]), cpu(s["dt"]))
+        t_next, n_act = h.next_block()
+        assert t_next == t_ref and n_act == len(act_ref)
+        assert np.array_equal(cpu(h.active()), act_ref)
+        h.predict(t_next)
+        h.force_jerk(None)
+        h.correct_and_timestep()
+    h.close()
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (2, 16384), (3, 4096), (4, 6000), (5, 2047)])
+def test_first_100_block_steps_bit_exact_schedule(gd, cfg, n):
+    # north_star: active-set and block-time-step indices bit-exact over the first 100 block steps
+    w = W.config(cfg, n=n)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    for k in range(100):
+        t_next, n_act = h.next_block()
+        act = cpu(h.active())
+        h.predict(t_next)
+        h.force_jerk(None)
+        h.correct_and_timestep()
+        o.step()
+        assert t_next == o.t and np.array_equal(act, o.active), f"step {k}"
+    s = {k: cpu(v) for k, v in h.state(("x", "t", "dt")).items()}
+    assert np.array_equal(s["t"], o.t_i) and np.array_equal(s["dt"], o.dt)
+    assert np.abs(s["x"] - o.x).max() < 1e-12
+    hist, diag = h.level_histogram()
+    assert np.array_equal(hist, o.level_hist) and diag[0] == o.nan_count and diag[1] == o.dtmin_clamps
+    assert h.block_steps == 100 and h.particle_steps == o.particle_steps
+    assert o.min_margin > 1e-10, "a time-step decision sat on a threshold: bit-exactness would be luck"
+    h.close()
+
+
+# ---------------------------------------------------------------------------------------------- energy
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (4, 3001), (5, 4096)])
+def test_energy_matches_oracle(gd, cfg, n):
+    w = W.config(cfg, n=n)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    K, U = h.energy()
+    K_ref, U_ref = oracle.energy(w.m, w.x, w.v, w.eps)
+    assert abs(K / K_ref - 1) < 1e-13 and abs(U / U_ref - 1) < 1e-13
+    h.close()
+
+
+def test_energy_off_sync_uses_predicted_state(gd):
+    w = W.config(1, n=512)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    h.step(37)
+    o.run(max_steps=37)
+    K, U = h.energy()
+    K_ref, U_ref = o.energy()
+    assert abs(K / K_ref - 1) < 1e-11 and abs(U / U_ref - 1) < 1e-11
+    h.close()
+
+
+def test_c1_integration_energy_error_matches_oracle(gd):
+    # C1: integrate to t = 0.125; same schedule statistics; |dE/E| within 10 % of the oracle's (north_star),
+    # with an absolute floor at the rounding level of E itself (|dE/E| ~ 1e-9 here is ~1e7 ulp: well resolved)
+    w = W.config(1)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    K0, U0 = h.energy()
+    K0r, U0r = o.energy()
+    steps, psteps = h.run_until(w.t_end)
+    o.run(w.t_end)
+    assert h.t == o.t == w.t_end
+    assert steps == o.block_steps and psteps == o.particle_steps
+    K, U = h.energy()
+    Kr, Ur = o.energy()
+    de = abs((K + U) / (K0 + U0) - 1)
+    de_ref = abs((Kr + Ur) / (K0r + U0r) - 1)
+    assert abs(de - de_ref) <= 0.1 * de_ref + 1e-13, (de, de_ref)
+    h.close()
+
+
+# ----------------------------------------------------------------------------------------- edge cases
+def test_single_particle_and_two_body(gd):
+    z = np.zeros((1, 3))
+    h = gd.Hermite(np.array([1.0]), z, np.array([[1.0, 0, 0]]), 1e-4, 0.01)
+    assert cpu(h.state(("dt",))["dt"])[0] == 0.125
+    h.run_until(0.5)
+    s = h.state_host(("x", "a"))
+    assert h.block_steps == 4 and np.allclose(s["x"][0], [0.5, 0, 0], atol=1e-16) and not s["a"].any()
+    h.close()
+    w = W.two_body(0.5, 0.5, 1.0, 0.0)
+    h = gd.Hermite(w.m, w.x, w.v, 0.0, 0.01)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, 0.0, 0.01)
+    h.run_until(1.0)
+    o.run(1.0)
+    assert h.block_steps == o.block_steps
+    assert np.abs(h.state_host(("x",))["x"] - o.x).max() < 1e-14
+    h.close()
+
+
+def test_errors_are_reported(gd):
+    w = W.config(1, n=64)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    with pytest.raises(gd.GravidyError) as e:
+        h.correct_and_timestep()
+    assert e.value.code == gd.GD_ESTATE
+    with pytest.raises(gd.GravidyError):
+        h.set_option("no_such_key", 1)
+    with pytest.raises(gd.GravidyError) as e:
+        gd.Hermite(w.m, w.x, w.v, w.eps, -1.0)
+    assert e.value.code == gd.GD_EINVAL
+    h.close()
+
+
+def test_host_init_equals_device_init(gd):
+    w = W.config(4, n=1500)
+    h1 = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h2 = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta, host=True)
+    h1.step(5)
+    h2.step(5)
+    s1, s2 = h1.state_host(), h2.state_host()
+    for k in s1:
+        assert np.array_equal(s1[k], s2[k]), k
+    h1.close()
+    h2.close()
