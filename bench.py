@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- the Hermite block-step hot path on synthetic Plummer clusters (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C2]
+
+One STEP = one pass of the whole hot path over the workload:
+    gd_init (a0: all-active force+jerk, initial dt)  ->  gd_energy (a6)
+    -> block steps until t_end: gd_next_block (a1), gd_predict (a2), gd_force_jerk (a3/a4),
+       gd_correct_and_timestep (a5)  ->  gd_energy (a6)
+Default workload: BASELINE.json configs[1] = C2, Plummer sphere N = 16384, eps = 1e-4, eta = 0.01, to t = 1.
+
+metric  = FP64 Hermite force+jerk pair interactions per second (n_act * N per force call, N * N for init);
+value   = inputs resident in HBM when the timed region starts;  e2e = same through HOST buffers
+          (gd_init_host: H2D of m, x, v inside; gd_get_state_host: D2H of x, v inside).
+roofline = the force kernel that took most of the step's time, timed per launch with CUDA events by the library
+          ("profile" option) inside the timed region; bound "alu" (plain FP64 FMA pipe, 60 flop per pair).
+cpu_baseline / --impl reference = the CPU oracle (oracle/) on the box's host cores, on a bounded sample.
+
+Multi-GPU: the path does not shard in this build (north_star: one GPU) -- "replicas only": every rank runs an
+independent replica of the workload; value = sum over ranks / max time over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+FLOP_PER_PAIR = 60.0                      # BASELINE.json convention
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x DFMA lanes/clk/SM x 2 flop x max SM clock = 37.2
+METRIC = "fp64_hermite_force_jerk_interactions_per_s"
+UNIT = "interactions/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C2", help="C1..C5 (BASELINE.json configs); default C2 = configs[1]")
+    ap.add_argument("--n", type=int, default=None, help="override the particle count (experiments only)")
+    ap.add_argument("--t-end", type=float, default=None, help="override the end time (experiments only)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the C3 force-kernel sweep (extra key)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    return ap.parse_args()
+
+
+def load_workload(args):
+    from paper_1702_00440_b200 import workloads as W
+    k = int(args.workload.lstrip("Cc"))
+    w = W.config(k, n=args.n)
+    t_end = args.t_end if args.t_end is not None else w.t_end
+    if t_end <= 0.0:
+        t_end = 2.0 ** -7                 # C3/C5 name no end time: 10-ish block steps' worth
+    return w, t_end
+
+
+# ------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            self.thread.join(timeout=2)
+
+    def summary(self) -> dict:
+        sm, mx, reasons = [], 0.0, set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = max(mx, float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, flag in zip(names, r[3:7]):
+                if flag.lower().startswith("active"):
+                    reasons.add(name)
+        busy = [c for c in sm if c > 0.5 * mx] or sm
+        return {"sm_mhz": statistics.median(busy) if busy else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------ our arm
+def run_step(gd, m, x, v, w, t_end, host: bool, profile: bool):
+    """One pass of the whole hot path.  host=False: m, x, v are CUDA tensors; host=True: pinned numpy arrays,
+    and the final state comes back to host arrays (gd_get_state_host)."""
+    h = gd.Hermite(m, x, v, w.eps, w.eta, host=host)
+    if profile:
+        h.set_option("profile", 1)
+    k0, u0 = h.energy()
+    steps, psteps = h.run_until(t_end)
+    k1, u1 = h.energy()
+    out = {"n": w.n, "block_steps": steps, "particle_steps": psteps, "e0": k0 + u0, "e1": k1 + u1,
+           "interactions": float(w.n) * w.n + float(psteps) * w.n, "t": h.t}
+    if host:
+        s = h.state_host(("x", "v"))
+        out["d2h_bytes"] = s["x"].nbytes + s["v"].nbytes + 4 * 8       # state + two (K, U) pairs
+        out["h2d_bytes"] = 7 * 8 * w.n
+    if profile:
+        out["prof"] = h.profile()
+    out["launches"] = h.kernel_launches
+    h.close()
+    return out
+
+
+def flush_l2(torch, buf):
+    buf.add_(1)                            # 256 MiB read + write: larger than the 126 MB L2
+
+
+def force_sweep(gd, torch, W):
+    """C3: isolated gd_force_jerk at N = 65536 over n_act in {1, 16, 256, 4096, 65536} (extra key, not `value`)."""
+    w = W.config(3)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h.predict(0.0)
+    rows = []
+    for n_act in (1, 16, 256, 4096, 65536):
+        idx = torch.from_numpy(W.active_indices(w.n, n_act)).cuda()
+        a = torch.empty((n_act, 3), dtype=torch.float64, device="cuda")
+        j = torch.empty_like(a)
+        for _ in range(3):
+            h.force_jerk(idx, a, j)
+        reps = 200 if n_act <= 4096 else 10
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            h.force_jerk(idx, a, j)
+        e1.record()
+        torch.cuda.synchronize()
+        sec = e0.elapsed_time(e1) * 1e-3 / reps
+        rate = n_act * w.n / sec
+        rows.append({"n_act": n_act, "kernel": h.last_force_kernel, "us": round(sec * 1e6, 2),
+                     "interactions_per_s": rate, "tflops60": rate * FLOP_PER_PAIR / 1e12,
+                     "frac_fp64_nominal": rate * FLOP_PER_PAIR / 1e12 / FP64_NOMINAL_TFLOPS})
+    h.close()
+    return {"workload": "C3 Plummer N=65536, back-to-back launches (state L2-resident)", "points": rows}
+
+
+def cpu_sample_steps(n: int) -> int:
+    """Block steps in the oracle's bounded sample: about 10-20 s of host work for C2 on 8 cores."""
+    return int(min(4096, max(64, (1 << 24) // n)))
+
+
+def cpu_baseline(w, t_end):
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload: INIT (all-active pair
+    sums, initial dt) + the first cpu_sample_steps(N) block steps (not past t_end), plain sequential FP64 accumulation."""
+    import oracle
+    t0 = time.perf_counter()
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta, acc_mode="plain")
+    o.run(t_end, max_steps=cpu_sample_steps(w.n))
+    sec = time.perf_counter() - t0
+    pairs = float(w.n) * w.n + float(o.particle_steps) * w.n
+    return {"value": pairs / sec, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{w.name}: INIT (N^2 pairs) + first {o.block_steps} block steps "
+                      f"({o.particle_steps} particle steps, to t={o.t:.6g}); plain FP64 sums; {sec:.1f} s"}, sec
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def main_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_1702_00440_b200 import binding as gd, workloads as W
+    gd.load()
+    w, t_end = load_workload(args)
+
+    # device-resident and pinned-host copies of the inputs
+    m_d, x_d, v_d = (torch.from_numpy(u).cuda() for u in (w.m, w.x, w.v))
+    m_h, x_h, v_h = (torch.from_numpy(u).pin_memory().numpy() for u in (w.m, w.x, w.v))
+    l2buf = torch.zeros(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        run_step(gd, m_d, x_d, v_d, w, t_end, host=False, profile=True)
+    run_step(gd, m_h, x_h, v_h, w, t_end, host=True, profile=False)
+
+    # ---- timed region: K steps, inputs resident in HBM, L2 flushed between steps ----
+    results = []
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        e0.record()
+        for _ in range(args.steps):
+            flush_l2(torch, l2buf)
+            results.append(run_step(gd, m_d, x_d, v_d, w, t_end, host=False, profile=True))
+        e1.record()
+        barrier()
+    sec = e0.elapsed_time(e1) * 1e-3
+    # ---- end to end: K steps through host buffers (H2D of inputs and D2H of the state inside) ----
+    e2e_results = []
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        flush_l2(torch, l2buf)
+        e2e_results.append(run_step(gd, m_h, x_h, v_h, w, t_end, host=True, profile=False))
+    barrier()
+    sec_e2e = time.perf_counter() - t0
+
+    if world > 1:
+        tt = torch.tensor([sec, sec_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        sec, sec_e2e = tt.tolist()
+    pairs = sum(r["interactions"] for r in results) * world          # replicas: identical work on every rank
+    pairs_e2e = sum(r["interactions"] for r in e2e_results) * world
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    return finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, sec_e2e, pairs, pairs_e2e,
+                       clocks.summary())
+
+
+# dram bytes per launch of the dominant force kernel from the committed `ncu --set full` capture under profiles/
+# (None until one exists for the workload; see profiles/README.md)
+NCU_TRAFFIC_BYTES = {}
+
+
+def finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, sec_e2e, pairs, pairs_e2e, clocks):
+    K = args.steps
+    prof = {k: {f: sum(r["prof"][k][f] for r in results) for f in ("launches", "ms", "pairs")} for k in ("ipar", "jsplit")}
+    dom = max(prof, key=lambda k: prof[k]["ms"])
+    d = prof[dom]
+    achieved = FLOP_PER_PAIR * d["pairs"] / (d["ms"] * 1e-3) / 1e12 if d["ms"] > 0 else 0.0
+    peak_probe, _ = gd.fp64_peak_probe(1 << 16)
+    roofline = {
+        "bound": "alu", "kernel": {"ipar": "k_force_ipar", "jsplit": "k_force_jsplit"}[dom],
+        "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
+        "traffic": NCU_TRAFFIC_BYTES.get((args.workload, dom)),
+        "peak_source": "derived: 148 SM x 64 DFMA lanes/clk x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
+                       "entry); register-only DFMA probe on this box: %.2f TFLOP/s" % (peak_probe / 1e12),
+        "launches": int(d["launches"]), "avg_launch_us": 1e3 * d["ms"] / max(d["launches"], 1),
+        "flop_per_launch": FLOP_PER_PAIR * d["pairs"] / max(d["launches"], 1),
+        "share_of_step": d["ms"] * 1e-3 / sec,
+        "by_kernel": {k: {"launches": int(v["launches"]), "ms": v["ms"],
+                          "tflops60": (FLOP_PER_PAIR * v["pairs"] / (v["ms"] * 1e-3) / 1e12) if v["ms"] > 0 else 0.0}
+                      for k, v in prof.items()},
+    }
+    r0 = results[-1]
+    value = pairs / sec
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": 1e3 * sec / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: {w.name}, eps={w.eps}, eta={w.eta}, init + block steps to t={t_end} "
+                               "+ energy at both ends", "n": w.n, "t_end": t_end,
+                   "l2": "256 MiB buffer rewritten between steps (flush); inside a step the %.1f MB state is "
+                         "L2-resident by construction" % (184e-6 * w.n),
+                   "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (path does not shard)"},
+        "clocks": clocks,
+        "e2e": {"value": pairs_e2e / sec_e2e, "unit": UNIT,
+                "h2d_bytes_per_step": e2e_results[-1]["h2d_bytes"], "d2h_bytes_per_step": e2e_results[-1]["d2h_bytes"],
+                "ms_per_step": 1e3 * sec_e2e / K},
+        "gpu_launches": int(sum(r["launches"] for r in results)),
+        "roofline": roofline,
+        "tflops60": value * FLOP_PER_PAIR / 1e12,
+        "frac_fp64_nominal": value * FLOP_PER_PAIR / 1e12 / FP64_NOMINAL_TFLOPS,
+        "wall_s_per_nbody_time_unit": (sec / K) / t_end,
+        "block_steps": r0["block_steps"], "particle_steps": r0["particle_steps"],
+        "mean_n_act": r0["particle_steps"] / max(r0["block_steps"], 1),
+        "energy": {"e0": r0["e0"], "e1": r0["e1"], "rel_err": abs(r0["e1"] / r0["e0"] - 1.0)},
+    }
+    if not args.no_sweep:
+        line["force_sweep"] = force_sweep(gd, torch, W)
+    if not args.no_cpu and world == 1:
+        line["cpu_baseline"], _ = cpu_baseline(w, t_end)
+    print(json.dumps(line), flush=True)
+    return line
+
+
+# ---------------------------------------------------------------------------------------- reference arm
+def main_reference(args):
+    """The oracle as it stands, timed on the host cores: each step = the bounded sample of cpu_baseline()."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    w, t_end = load_workload(args)
+    for _ in range(min(args.warmup, 1)):              # a CPU program needs no more than one warm-up pass
+        cpu_baseline(w, t_end)
+    secs, vals, info = 0.0, [], None
+    for _ in range(args.steps):
+        info, s = cpu_baseline(w, t_end)
+        secs += s
+        vals.append(info["value"])
+    value = sum(vals) / len(vals)
+    info = dict(info, value=value)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: {w.name}, eps={w.eps}, eta={w.eta}; bounded sample per step: "
+                                   f"INIT + first {cpu_sample_steps(w.n)} block steps", "n": w.n, "t_end": t_end},
+            "cpu_baseline": info,
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        main_reference(a)
+    else:
+        main_ours(a)

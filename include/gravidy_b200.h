@@ -82,7 +82,8 @@ GD_API const char *gd_last_error(const gd_ctx *ctx);
 
 /* Tunables.  key: "jsplit_max_nact" (active sets of at most this size use the j-split kernel; default 2048),
  * "dt_level_min", "dt_level_max" (override GD_LEVEL_MIN/MAX before the first step; 0 <= min <= max <= 52),
- * "halving_mode" (0: one halving per step [default]; 1: halve until dt <= dt_req).  GD_EINVAL on unknown keys. */
+ * "halving_mode" (0: one halving per step [default]; 1: halve until dt <= dt_req),
+ * "profile" (0/1: time every force launch with CUDA events, see gd_get_profile).  GD_EINVAL on unknown keys. */
 GD_API int gd_set_option(gd_ctx *ctx, const char *key, double value);
 
 /* Step (v).  t_next = min_i (t_i + dt_i); the active list becomes { i ascending : t_i + dt_i == t_next }
@@ -153,6 +154,14 @@ GD_API int gd_get_active(gd_ctx *ctx, int32_t *idx_dev, int64_t cap);
 /* Particle steps taken per level k (dt = 2^-k) since init -> counts_host[64]; and diagnostic counters
  * diag_host[2] = { time-step criteria that evaluated to NaN, clamps at dt_min }.  Synchronises. */
 GD_API int gd_get_level_histogram(gd_ctx *ctx, int64_t *counts_host, int64_t *diag_host);
+
+/* Optional CUDA-event timing of the force launches, switched on with gd_set_option(ctx, "profile", 1): every
+ * gd_force_jerk issued afterwards is bracketed by two events on the context's stream (the all-active evaluation
+ * inside gd_init runs before the option can be set and is not timed).  prof_host[12] receives, for kind k = 0
+ * (i-parallel kernel), 1 (j-split kernel + its cross-cluster combine), 2 (reserved):
+ *   prof[4k] launches timed, prof[4k+1] sum of durations in ms, prof[4k+2] sum of pair interactions (n_act * n),
+ *   prof[4k+3] sum of squared durations (ms^2).  Synchronises on the last recorded event. */
+GD_API int gd_get_profile(gd_ctx *ctx, double *prof_host);
 
 /* Register-only DFMA loop on every SM: measures the FP64 peak the force kernels are bounded by.  Returns the
  * achieved rate in flop/s (2 flop per FMA per lane) in *flops_host; ms_host receives the elapsed milliseconds.

@@ -48,6 +48,7 @@ SYMBOLS = {
     "gd_get_predicted": (_int, [_vp, _vp, _vp]),
     "gd_get_active": (_int, [_vp, _vp, _i64]),
     "gd_get_level_histogram": (_int, [_vp, _vp, _vp]),
+    "gd_get_profile": (_int, [_vp, _vp]),
     "gd_fp64_peak_probe": (_int, [_int, _pdbl, _pdbl]),
 }
 
@@ -281,6 +282,13 @@ class Hermite:
         idx = torch.empty((max(k, 1),), dtype=torch.int32, device="cuda")
         self._check(self._lib.gd_get_active(self._h, idx.data_ptr(), idx.shape[0]))
         return idx[:k]
+
+    def profile(self) -> dict:
+        """Event-timed force launches since the "profile" option was set: per kernel launches, ms, pairs."""
+        p = np.zeros(12)
+        self._check(self._lib.gd_get_profile(self._h, p.ctypes.data))
+        return {k: {"launches": int(p[4 * i]), "ms": float(p[4 * i + 1]), "pairs": float(p[4 * i + 2]),
+                    "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit"))}
 
     def level_histogram(self) -> tuple[np.ndarray, np.ndarray]:
         h, d = np.zeros(64, dtype=np.int64), np.zeros(2, dtype=np.int64)

@@ -23,6 +23,48 @@ static int gd_fail(gd_ctx *c, int code, const char *msg)
     return code;
 }
 
+// ---- optional event timing of the force launches ---------------------------------------------------------
+int gd_prof_drain(gd_ctx *c)
+{
+    if (c->ev_pending == 0) return 0;
+    GD_CUDA(c, cudaEventSynchronize(c->ev1[c->ev_pending - 1]));
+    for (int k = 0; k < c->ev_pending; ++k) {
+        float ms = 0.f;
+        GD_CUDA(c, cudaEventElapsedTime(&ms, c->ev0[k], c->ev1[k]));
+        double *p = c->prof + 4 * c->ev_kind[k];
+        p[0] += 1.0;
+        p[1] += ms;
+        p[2] += c->ev_pairs[k];
+        p[3] += (double)ms * ms;
+    }
+    c->ev_pending = 0;
+    return 0;
+}
+
+int gd_prof_begin(gd_ctx *c)
+{
+    if (!c->profile) return -1;
+    if (!c->ev_created) {
+        for (int k = 0; k < GD_PROF_POOL; ++k) {
+            if (cudaEventCreate(&c->ev0[k]) != cudaSuccess || cudaEventCreate(&c->ev1[k]) != cudaSuccess) return -1;
+        }
+        c->ev_created = true;
+    }
+    if (c->ev_pending == GD_PROF_POOL && gd_prof_drain(c)) return -1;
+    int slot = c->ev_pending;
+    if (cudaEventRecord(c->ev0[slot], c->stream) != cudaSuccess) return -1;
+    return slot;
+}
+
+void gd_prof_end(gd_ctx *c, int slot, int kind, double pairs)
+{
+    if (slot < 0) return;
+    cudaEventRecord(c->ev1[slot], c->stream);
+    c->ev_kind[slot] = kind;
+    c->ev_pairs[slot] = pairs;
+    c->ev_pending = slot + 1;
+}
+
 // ---- workspace -------------------------------------------------------------------------------------------
 static inline int64_t gd_pad(int64_t n) { return ((n + GD_TILE_J - 1) / GD_TILE_J) * GD_TILE_J; }
 static inline int64_t gd_pcap(int64_t np) { return (4 * np > (1 << 20)) ? 4 * np : (1 << 20); }
@@ -84,6 +126,8 @@ extern "C" void gd_destroy(gd_ctx *ctx)
 {
     if (!ctx) return;
     if (ctx->h_cell) cudaFreeHost(ctx->h_cell);
+    if (ctx->ev_created)
+        for (int k = 0; k < GD_PROF_POOL; ++k) { cudaEventDestroy(ctx->ev0[k]); cudaEventDestroy(ctx->ev1[k]); }
     free(ctx);
 }
 
@@ -175,6 +219,11 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
 {
     if (!c || !key) return GD_EINVAL;
     if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; return GD_OK; }
+    if (!strcmp(key, "profile")) {
+        int rc = gd_prof_drain(c);
+        c->profile = (int)value;
+        return rc;
+    }
     if (!strcmp(key, "halving_mode")) { c->halving_mode = value != 0.0; return GD_OK; }
     if (!strcmp(key, "dt_level_min") || !strcmp(key, "dt_level_max")) {
         int lv = (int)value;
@@ -370,6 +419,15 @@ extern "C" int gd_get_active(gd_ctx *c, int32_t *idx_dev, int64_t cap)
     if (cap < c->n_act) return gd_fail(c, GD_EINVAL, "gd_get_active: capacity too small");
     if (c->n_act > 0)
         GD_CUDA(c, cudaMemcpyAsync(idx_dev, c->d.idx, c->n_act * sizeof(int32_t), cudaMemcpyDeviceToDevice, c->stream));
+    return GD_OK;
+}
+
+extern "C" int gd_get_profile(gd_ctx *c, double *prof_host)
+{
+    if (!c || !prof_host) return GD_EINVAL;
+    int rc = gd_prof_drain(c);
+    if (rc) return rc;
+    memcpy(prof_host, c->prof, sizeof c->prof);
     return GD_OK;
 }
 

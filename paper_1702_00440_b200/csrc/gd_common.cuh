@@ -34,6 +34,7 @@ struct gd_dev {
 };
 
 #define GD_SCAN_MAX_BLOCKS 1024
+#define GD_PROF_POOL 64
 #define GD_SCAN_THREADS 1024
 
 struct gd_ctx {
@@ -54,8 +55,20 @@ struct gd_ctx {
     int last_force_kernel;
     unsigned int epoch, ticket_min_base, ticket_cmp_base;
     int sm_count;
+    // optional CUDA-event timing of the force launches ("profile" option; see gd_get_profile)
+    int profile;
+    cudaEvent_t ev0[GD_PROF_POOL], ev1[GD_PROF_POOL];
+    double ev_pairs[GD_PROF_POOL];
+    int ev_kind[GD_PROF_POOL];
+    int ev_pending;
+    bool ev_created;
+    double prof[12];             // per kind k = 0 (i-parallel), 1 (j-split), 2 (other stages): {launches, ms, pairs, ms^2}
     char err[512];
 };
+
+int gd_prof_begin(gd_ctx *c);                               // gd_api.cu: record the start event (returns slot or -1)
+void gd_prof_end(gd_ctx *c, int slot, int kind, double pairs);
+int gd_prof_drain(gd_ctx *c);
 
 // ---- launch wrappers (one per kernel file); all enqueue on c->stream and bump c->launches -------------
 int gdk_pack_state(gd_ctx *c, const double *m, const double *x, const double *v);           // gd_predict.cu

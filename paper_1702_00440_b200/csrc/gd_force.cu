@@ -393,6 +393,9 @@ static int gd_force_jsplit(gd_ctx *c, const int32_t *idx, int64_t n_act, double 
 int gdk_force(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out)
 {
     if (n_act <= 0) return 0;
-    if (n_act <= c->jsplit_max_nact) return gd_force_jsplit(c, idx, n_act, a_out, j_out);
-    return gd_force_ipar(c, idx, n_act, a_out, j_out);
+    const bool js = n_act <= c->jsplit_max_nact;
+    const int slot = gd_prof_begin(c);
+    int rc = js ? gd_force_jsplit(c, idx, n_act, a_out, j_out) : gd_force_ipar(c, idx, n_act, a_out, j_out);
+    gd_prof_end(c, slot, js ? 1 : 0, (double)n_act * (double)c->n);
+    return rc;
 }
