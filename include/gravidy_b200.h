@@ -82,7 +82,7 @@ GD_API const char *gd_last_error(const gd_ctx *ctx);
 
 /* Tunables.  key: "jsplit_max_nact" (active sets of at most this size use the j-split kernel; default 2048),
  * "dt_level_min", "dt_level_max" (override GD_LEVEL_MIN/MAX before the first step; 0 <= min <= max <= 52),
- * "halving_mode" (0: one halving per step [default]; 1: halve until dt <= dt_req),
+ * "halving_mode" (1: halve until dt <= dt_req [default]; 0: a single halving per step),
  * "profile" (0/1: time every force launch with CUDA events, see gd_get_profile).  GD_EINVAL on unknown keys. */
 GD_API int gd_set_option(gd_ctx *ctx, const char *key, double value);
 
@@ -118,7 +118,7 @@ GD_API int gd_force_jerk_host(int64_t n, const double *m_host, const double *x_h
  *   a2 = (-6 (a0 - a1) - h (4 j0 + 2 j1)) / h^2 ;  a3 = (12 (a0 - a1) + 6 h (j0 + j1)) / h^3
  *   x = xp + a2 h^4/24 + a3 h^5/120 ;  v = vp + a2 h^3/6 + a3 h^4/24 ;  a2e = a2 + h a3
  *   dt_req = sqrt( eta (|a1||a2e| + |j1|^2) / (|j1||a3| + |a2e|^2) )          (denominator 0 -> +inf)
- *   dt_i <- h/2 if dt_req < h ; 2h if dt_req >= 2h and t_next is a multiple of 2h ; else h ; clamped
+ *   dt_i <- h/2, h/4, ... (largest 2^-k h <= dt_req) if dt_req < h ; 2h if dt_req >= 2h and t_next is a multiple of 2h ; else h ; clamped
  *   a_i <- a1, jerk_i <- j1, t_i <- t_next.
  * GD_ESTATE unless preceded by next_block, predict(t_next) and force_jerk(NULL). */
 GD_API int gd_correct_and_timestep(gd_ctx *ctx);

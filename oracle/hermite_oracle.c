@@ -162,7 +162,8 @@ ORC_API void orc_initial_dt(int64_t n, const double *a, const double *j, double 
 }
 
 /* BLOCKUPDATE [reading R7]: h = current step, t_new = time just reached (multiple of h).
- *   dt_req <  h                         -> h/2   (halving_mode 1: keep halving while > dt_req)
+ *   dt_req <  h                         -> halving_mode 1 (default): h/2, h/4, ... until <= dt_req;
+ *                                          halving_mode 0 (variant): a single halving, h/2
  *   dt_req >= 2h and t_new mod 2h == 0  -> 2h
  *   otherwise                           -> h ;   then clamp to [dt_min, dt_max].  NaN -> keep h. */
 ORC_API double orc_block_update(double h, double dt_req, double t_new, double dt_min, double dt_max,

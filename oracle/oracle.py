@@ -142,7 +142,7 @@ def block_init(value: float, dt_min: float = DT_MIN, dt_max: float = DT_MAX) -> 
     return float(_load().orc_block_init(value, dt_min, dt_max))
 
 
-def block_update(h, dt_req, t_new, dt_min=DT_MIN, dt_max=DT_MAX, halving_mode=0) -> float:
+def block_update(h, dt_req, t_new, dt_min=DT_MIN, dt_max=DT_MAX, halving_mode=1) -> float:
     return float(_load().orc_block_update(h, dt_req, t_new, dt_min, dt_max, halving_mode))
 
 
@@ -170,7 +170,7 @@ def predict(t, x, v, a, j, t_i):
 
 
 def correct(active, t_new, eta, x, v, a, j, t_i, dt, xp, vp, a1, j1, dt_min=DT_MIN, dt_max=DT_MAX,
-            halving_mode=0):
+            halving_mode=1):
     """Corrector + time-step update for the active list; returns new copies (x, v, a, j, t_i, dt, dt_req)."""
     active = np.ascontiguousarray(active, dtype=np.int32)
     x, v, a, j, t_i, dt = (_f64(u).copy() for u in (x, v, a, j, t_i, dt))
@@ -195,7 +195,7 @@ def energy(m, x, v, eps):
 class HermiteOracle:
     """The whole integrator: INIT then block steps, state in numpy arrays owned here."""
 
-    def __init__(self, m, x, v, eps, eta, dt_min=DT_MIN, dt_max=DT_MAX, halving_mode=0,
+    def __init__(self, m, x, v, eps, eta, dt_min=DT_MIN, dt_max=DT_MAX, halving_mode=1,
                  acc_mode: str = "compensated"):
         self._lib = _load()
         self.m, self.x, self.v = _f64(m).copy(), _f64(x).copy(), _f64(v).copy()

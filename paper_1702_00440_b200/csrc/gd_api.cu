@@ -152,7 +152,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->lvl_max = GD_LEVEL_MAX;
     c->dt_max = ldexp(1.0, -GD_LEVEL_MIN);
     c->dt_min = ldexp(1.0, -GD_LEVEL_MAX);
-    c->halving_mode = 0;
+    c->halving_mode = 1;
     c->jsplit_max_nact = 2048;
     c->stream = (cudaStream_t)stream;
     gd_carve(&c->d, ws, c->np, c->pcap);

@@ -113,9 +113,9 @@ def test_block_init():
 
 def test_block_update():
     h = 2.0 ** -6
-    assert oracle.block_update(h, 0.9 * h, 5 * h) == h / 2                 # shrink: one halving
-    assert oracle.block_update(h, 0.1 * h, 5 * h) == h / 2                 # ... even if far below
-    assert oracle.block_update(h, 0.1 * h, 5 * h, halving_mode=1) == h / 16
+    assert oracle.block_update(h, 0.9 * h, 5 * h) == h / 2                 # shrink: one halving is enough
+    assert oracle.block_update(h, 0.1 * h, 5 * h) == h / 16                # default (R7): halve until dt <= dt_req
+    assert oracle.block_update(h, 0.1 * h, 5 * h, halving_mode=0) == h / 2 # variant: a single halving per step
     assert oracle.block_update(h, 1.5 * h, 4 * h) == h                     # keep
     assert oracle.block_update(h, 2.0 * h, 4 * h) == 2 * h                 # double only when commensurate
     assert oracle.block_update(h, 5.0 * h, 5 * h) == h
