@@ -83,6 +83,8 @@ GD_API const char *gd_last_error(const gd_ctx *ctx);
 /* Tunables.  key: "jsplit_max_nact" (active sets of at most this size use the j-split kernel; default 2048),
  * "dt_level_min", "dt_level_max" (override GD_LEVEL_MIN/MAX before the first step; 0 <= min <= max <= 52),
  * "halving_mode" (1: halve until dt <= dt_req [default]; 0: a single halving per step),
+ * "ipar_variant" (-1 automatic [default]; 0..3 force the i-parallel tile shape), "ipar_split" (0 automatic; > 0
+ * force the number of source splits) -- tuning experiments only,
  * "profile" (0/1: time every force launch with CUDA events, see gd_get_profile).  GD_EINVAL on unknown keys. */
 GD_API int gd_set_option(gd_ctx *ctx, const char *key, double value);
 
@@ -142,6 +144,9 @@ GD_API int64_t gd_block_steps(const gd_ctx *ctx);       /* "Iter"   of Listing 1
 GD_API int64_t gd_particle_steps(const gd_ctx *ctx);    /* "Nsteps" of Listing 1 */
 GD_API int     gd_last_force_kernel(const gd_ctx *ctx); /* 0 none, 1 i-parallel, 2 j-split */
 GD_API int64_t gd_kernel_launches(const gd_ctx *ctx);   /* kernels launched on behalf of this ctx so far */
+/* Launch geometry of the last force evaluation -> geom_host[4] = { kernel variant, i-tiles (i-parallel) or sink
+ * groups (j-split), source splits, source units (of 64 records) per split }.  Diagnostics only. */
+GD_API int gd_last_force_geometry(const gd_ctx *ctx, int *geom_host);
 
 /* Copies of the state into DEVICE arrays ([n,3] or [n]); any pointer may be NULL.  Asynchronous. */
 GD_API int gd_get_state(gd_ctx *ctx, double *x_dev, double *v_dev, double *a_dev, double *j_dev, double *t_dev, double *dt_dev);

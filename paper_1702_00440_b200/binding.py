@@ -43,6 +43,7 @@ SYMBOLS = {
     "gd_particle_steps": (_i64, [_vp]),
     "gd_last_force_kernel": (_int, [_vp]),
     "gd_kernel_launches": (_i64, [_vp]),
+    "gd_last_force_geometry": (_int, [_vp, _vp]),
     "gd_get_state": (_int, [_vp] * 7),
     "gd_get_state_host": (_int, [_vp] * 7),
     "gd_get_predicted": (_int, [_vp, _vp, _vp]),
@@ -251,6 +252,12 @@ class Hermite:
     @property
     def kernel_launches(self) -> int:
         return int(self._lib.gd_kernel_launches(self._h))
+
+    @property
+    def last_force_geometry(self) -> tuple:
+        g = (C.c_int * 4)()
+        self._check(self._lib.gd_last_force_geometry(self._h, g))
+        return tuple(g)
 
     def state(self, names=("x", "v", "a", "j", "t", "dt")) -> dict:
         """Copies of the state as CUDA tensors."""

@@ -101,6 +101,7 @@ static size_t gd_carve(gd_dev *d, void *base, int64_t np, int64_t pcap)
     t.blockmin = w.take<double>(GD_SCAN_MAX_BLOCKS);
     t.agg = w.take<unsigned long long>(GD_SCAN_MAX_BLOCKS);
     t.ticket = w.take<unsigned int>(4);
+    t.tile_ticket = w.take<unsigned int>(np / 32);
     t.cell = w.take<double>(4);
     t.hist = w.take<long long>(64);
     t.diag = w.take<long long>(2);
@@ -154,6 +155,11 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->dt_min = ldexp(1.0, -GD_LEVEL_MAX);
     c->halving_mode = 1;
     c->jsplit_max_nact = 2048;
+    c->ipar_variant = -1;
+    c->ipar_split = 0;
+    c->js_bi = 0;
+    c->js_cluster = 0;
+    c->js_ctas_per_sm = 2;
     c->stream = (cudaStream_t)stream;
     gd_carve(&c->d, ws, c->np, c->pcap);
     int dev = 0;
@@ -219,6 +225,11 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
 {
     if (!c || !key) return GD_EINVAL;
     if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; return GD_OK; }
+    if (!strcmp(key, "ipar_variant")) { c->ipar_variant = (int)value; return GD_OK; }
+    if (!strcmp(key, "ipar_split")) { c->ipar_split = (int)value; return GD_OK; }
+    if (!strcmp(key, "js_bi")) { c->js_bi = (int)value; return GD_OK; }
+    if (!strcmp(key, "js_cluster")) { c->js_cluster = (int)value; return GD_OK; }
+    if (!strcmp(key, "js_ctas_per_sm")) { c->js_ctas_per_sm = (int)value < 1 ? 1 : (int)value; return GD_OK; }
     if (!strcmp(key, "profile")) {
         int rc = gd_prof_drain(c);
         c->profile = (int)value;
@@ -368,6 +379,12 @@ extern "C" int64_t gd_block_steps(const gd_ctx *c) { return c ? c->block_steps :
 extern "C" int64_t gd_particle_steps(const gd_ctx *c) { return c ? c->particle_steps : 0; }
 extern "C" int gd_last_force_kernel(const gd_ctx *c) { return c ? c->last_force_kernel : 0; }
 extern "C" int64_t gd_kernel_launches(const gd_ctx *c) { return c ? c->launches : 0; }
+extern "C" int gd_last_force_geometry(const gd_ctx *c, int *geom_host)
+{
+    if (!c || !geom_host) return GD_EINVAL;
+    memcpy(geom_host, c->last_geom, sizeof c->last_geom);
+    return GD_OK;
+}
 
 extern "C" int gd_get_state(gd_ctx *c, double *x, double *v, double *a, double *j, double *t, double *dt)
 {

@@ -12,7 +12,8 @@
 #include <stdint.h>
 #include <stddef.h>
 
-#define GD_TILE_J 256            // sources per shared-memory tile of the i-parallel kernel; np is a multiple
+#define GD_TILE_J 256            // sources per shared-memory stage of the force kernels; np is a multiple
+#define GD_UNIT_J 64             // granularity of a CTA's source range (TMA copies stay 16-byte aligned)
 
 struct gd_dev {
     double4 *xm, *vt, *ad, *jk;
@@ -25,6 +26,7 @@ struct gd_dev {
     double *blockmin;            // [GD_SCAN_MAX_BLOCKS] per-block minima of tnext
     unsigned long long *agg;     // [GD_SCAN_MAX_BLOCKS] {epoch:32 | count:32} per-block aggregates of the compaction
     unsigned int *ticket;        // [4] monotonically increasing block tickets (never reset)
+    unsigned int *tile_ticket;   // [np / 32] arrivals per i-tile of a split force evaluation (re-armed to 0 by the last CTA)
     double *cell;                // [4] {t_next, n_act (as int64 bits), K, U}
     long long *hist;             // [64] particle steps per level
     long long *diag;             // [2]  NaN criteria, dt_min clamps
@@ -53,6 +55,9 @@ struct gd_ctx {
     double t_pred;
     int64_t block_steps, particle_steps, launches;
     int last_force_kernel;
+    int ipar_variant, ipar_split;        // tuning overrides (-1 / 0 = automatic)
+    int js_bi, js_cluster, js_ctas_per_sm;
+    int last_geom[4];                    // geometry of the last force launch: variant, i-tiles (or groups), splits, units per split
     unsigned int epoch, ticket_min_base, ticket_cmp_base;
     int sm_count;
     // optional CUDA-event timing of the force launches ("profile" option; see gd_get_profile)
