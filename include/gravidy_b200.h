@@ -80,11 +80,11 @@ GD_API void gd_destroy(gd_ctx *ctx);
 /* Text of the last error recorded on ctx (ctx == NULL: last error of a failed gd_init). Never NULL. */
 GD_API const char *gd_last_error(const gd_ctx *ctx);
 
-/* Tunables.  key: "jsplit_max_nact" (active sets of at most this size use the j-split kernel; default 2048),
+/* Tunables.  key: "jsplit_max_nact" (active sets of at most this size use the j-split kernel; default 512, capped
+ * at 32 x the number of clusters in its grid), "ipar_small_max_nact" (above that and up to this size the i-parallel
+ * kernel runs with 32-sink tiles, beyond it with 256-sink tiles; default 2048),
  * "dt_level_min", "dt_level_max" (override GD_LEVEL_MIN/MAX before the first step; 0 <= min <= max <= 52),
  * "halving_mode" (1: halve until dt <= dt_req [default]; 0: a single halving per step),
- * "ipar_variant" (-1 automatic [default]; 0..3 force the i-parallel tile shape), "ipar_split" (0 automatic; > 0
- * force the number of source splits) -- tuning experiments only,
  * "profile" (0/1: time every force launch with CUDA events, see gd_get_profile).  GD_EINVAL on unknown keys. */
 GD_API int gd_set_option(gd_ctx *ctx, const char *key, double value);
 
@@ -142,10 +142,10 @@ GD_API int64_t gd_n(const gd_ctx *ctx);
 GD_API int64_t gd_n_active(const gd_ctx *ctx);          /* size of the current internal active list */
 GD_API int64_t gd_block_steps(const gd_ctx *ctx);       /* "Iter"   of Listing 1 */
 GD_API int64_t gd_particle_steps(const gd_ctx *ctx);    /* "Nsteps" of Listing 1 */
-GD_API int     gd_last_force_kernel(const gd_ctx *ctx); /* 0 none, 1 i-parallel, 2 j-split */
+GD_API int     gd_last_force_kernel(const gd_ctx *ctx); /* 0 none, 1 i-parallel (256-sink tiles), 2 j-split, 3 i-parallel (32-sink tiles) */
 GD_API int64_t gd_kernel_launches(const gd_ctx *ctx);   /* kernels launched on behalf of this ctx so far */
-/* Launch geometry of the last force evaluation -> geom_host[4] = { kernel variant, i-tiles (i-parallel) or sink
- * groups (j-split), source splits, source units (of 64 records) per split }.  Diagnostics only. */
+/* Launch geometry of the last explicit force evaluation -> geom_host[4] = { kernel (as above, 0 = 256-sink tiles),
+ * i-tiles, source splits (i-parallel) or clusters per i-tile (j-split), units of 64 sources per split }.  Diagnostics only. */
 GD_API int gd_last_force_geometry(const gd_ctx *ctx, int *geom_host);
 
 /* Copies of the state into DEVICE arrays ([n,3] or [n]); any pointer may be NULL.  Asynchronous. */
@@ -163,7 +163,7 @@ GD_API int gd_get_level_histogram(gd_ctx *ctx, int64_t *counts_host, int64_t *di
 /* Optional CUDA-event timing of the force launches, switched on with gd_set_option(ctx, "profile", 1): every
  * gd_force_jerk issued afterwards is bracketed by two events on the context's stream (the all-active evaluation
  * inside gd_init runs before the option can be set and is not timed).  prof_host[12] receives, for kind k = 0
- * (i-parallel kernel), 1 (j-split kernel + its cross-cluster combine), 2 (reserved):
+ * (i-parallel kernel, 256-sink tiles), 1 (j-split kernel), 2 (i-parallel kernel, 32-sink tiles):
  *   prof[4k] launches timed, prof[4k+1] sum of durations in ms, prof[4k+2] sum of pair interactions (n_act * n),
  *   prof[4k+3] sum of squared durations (ms^2).  Synchronises on the last recorded event. */
 GD_API int gd_get_profile(gd_ctx *ctx, double *prof_host);

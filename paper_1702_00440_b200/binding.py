@@ -174,11 +174,16 @@ class Hermite:
             raise GravidyError(rc, self._lib.gd_last_error(self._h).decode())
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h.value:
-            self._lib.gd_destroy(self._h)
-            self._h = _vp(None)
+        h, lib = getattr(self, "_h", None), getattr(self, "_lib", None)
+        if h is not None and h.value and lib is not None:
+            lib.gd_destroy(h)
+            self._h = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:        # interpreter shutdown: ctypes may already be torn down
+            pass
 
     def set_option(self, key: str, value: float):
         self._check(self._lib.gd_set_option(self._h, key.encode(), float(value)))
@@ -247,7 +252,7 @@ class Hermite:
 
     @property
     def last_force_kernel(self) -> str:
-        return {0: "none", 1: "ipar", 2: "jsplit"}[int(self._lib.gd_last_force_kernel(self._h))]
+        return {0: "none", 1: "ipar", 2: "jsplit", 3: "ipar_small"}[int(self._lib.gd_last_force_kernel(self._h))]
 
     @property
     def kernel_launches(self) -> int:
@@ -295,7 +300,7 @@ class Hermite:
         p = np.zeros(12)
         self._check(self._lib.gd_get_profile(self._h, p.ctypes.data))
         return {k: {"launches": int(p[4 * i]), "ms": float(p[4 * i + 1]), "pairs": float(p[4 * i + 2]),
-                    "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit"))}
+                    "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit", "ipar_small"))}
 
     def level_histogram(self) -> tuple[np.ndarray, np.ndarray]:
         h, d = np.zeros(64, dtype=np.int64), np.zeros(2, dtype=np.int64)

@@ -102,6 +102,9 @@ static size_t gd_carve(gd_dev *d, void *base, int64_t np, int64_t pcap)
     t.agg = w.take<unsigned long long>(GD_SCAN_MAX_BLOCKS);
     t.ticket = w.take<unsigned int>(4);
     t.tile_ticket = w.take<unsigned int>(np / 32);
+    t.work = w.take<unsigned int>(4);
+    t.geom_s = w.take<int2>(np / 32 + 2);
+    t.geom_l = w.take<int2>(np / 256 + 2);
     t.cell = w.take<double>(4);
     t.hist = w.take<long long>(64);
     t.diag = w.take<long long>(2);
@@ -127,6 +130,8 @@ extern "C" void gd_destroy(gd_ctx *ctx)
 {
     if (!ctx) return;
     if (ctx->h_cell) cudaFreeHost(ctx->h_cell);
+    free(ctx->h_geom_s);
+    free(ctx->h_geom_l);
     if (ctx->ev_created)
         for (int k = 0; k < GD_PROF_POOL; ++k) { cudaEventDestroy(ctx->ev0[k]); cudaEventDestroy(ctx->ev1[k]); }
     free(ctx);
@@ -154,12 +159,8 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->dt_max = ldexp(1.0, -GD_LEVEL_MIN);
     c->dt_min = ldexp(1.0, -GD_LEVEL_MAX);
     c->halving_mode = 1;
-    c->jsplit_max_nact = 2048;
-    c->ipar_variant = -1;
-    c->ipar_split = 0;
-    c->js_bi = 0;
-    c->js_cluster = 0;
-    c->js_ctas_per_sm = 2;
+    c->jsplit_max_nact = 512;
+    c->ipar_small_max_nact = 2048;
     c->stream = (cudaStream_t)stream;
     gd_carve(&c->d, ws, c->np, c->pcap);
     int dev = 0;
@@ -175,13 +176,20 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     return GD_OK;
 }
 
-static int gd_init_common(gd_ctx *c, const double *m_dev, const double *x_dev, const double *v_dev)
+// scan scratch, tickets, histogram, diagnostics start from zero (epoch 0 = "never written"); then the launch
+// shapes and geometry tables of the force kernels
+static int gd_prepare(gd_ctx *c)
 {
-    // scan scratch, histogram, diagnostics start from zero (epoch 0 = "never written")
     GD_CUDA(c, cudaMemsetAsync(c->d.blockmin, 0, (char *)c->d.phi - (char *)c->d.blockmin, c->stream));
     c->epoch = 0;
     c->ticket_min_base = c->ticket_cmp_base = 0;
+    return gdk_force_setup(c);
+}
+
+static int gd_init_common(gd_ctx *c, const double *m_dev, const double *x_dev, const double *v_dev)
+{
     int rc;
+    if ((rc = gd_prepare(c))) return rc;
     if ((rc = gdk_pack_state(c, m_dev, x_dev, v_dev))) return rc;          // also the predicted records at t = 0
     c->t = 0.0;
     c->t_pred = 0.0;
@@ -225,11 +233,7 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
 {
     if (!c || !key) return GD_EINVAL;
     if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; return GD_OK; }
-    if (!strcmp(key, "ipar_variant")) { c->ipar_variant = (int)value; return GD_OK; }
-    if (!strcmp(key, "ipar_split")) { c->ipar_split = (int)value; return GD_OK; }
-    if (!strcmp(key, "js_bi")) { c->js_bi = (int)value; return GD_OK; }
-    if (!strcmp(key, "js_cluster")) { c->js_cluster = (int)value; return GD_OK; }
-    if (!strcmp(key, "js_ctas_per_sm")) { c->js_ctas_per_sm = (int)value < 1 ? 1 : (int)value; return GD_OK; }
+    if (!strcmp(key, "ipar_small_max_nact")) { c->ipar_small_max_nact = (int64_t)value; return GD_OK; }
     if (!strcmp(key, "profile")) {
         int rc = gd_prof_drain(c);
         c->profile = (int)value;
@@ -475,6 +479,7 @@ extern "C" int gd_force_jerk_host(int64_t n, const double *m_host, const double 
     if (e == cudaSuccess && idx_host && n_act > 0)
         e = cudaMemcpyAsync(c->d.idx, idx_host, n_act * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream);
     if (e != cudaSuccess) rc = gd_fail_cuda(c, e, "gd_force_jerk_host: H2D copy");
+    if (!rc) rc = gd_prepare(c);
     if (!rc) rc = gdk_pack_sources(c, st, st + c->np, st + 4 * c->np);
     if (!rc) rc = gdk_force(c, idx_host ? c->d.idx : nullptr, n_act, c->d.a1, c->d.j1);
     if (!rc && n_act > 0) {

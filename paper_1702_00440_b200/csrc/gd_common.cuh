@@ -27,6 +27,8 @@ struct gd_dev {
     unsigned long long *agg;     // [GD_SCAN_MAX_BLOCKS] {epoch:32 | count:32} per-block aggregates of the compaction
     unsigned int *ticket;        // [4] monotonically increasing block tickets (never reset)
     unsigned int *tile_ticket;   // [np / 32] arrivals per i-tile of a split force evaluation (re-armed to 0 by the last CTA)
+    unsigned int *work;          // [4] {next unit ticket, CTAs finished} of the persistent force grid (re-armed by the last CTA)
+    int2 *geom_s, *geom_l;       // [np / 32 + 2], [np / 256 + 2]: i-tiles -> {source splits, units per split}
     double *cell;                // [4] {t_next, n_act (as int64 bits), K, U}
     long long *hist;             // [64] particle steps per level
     long long *diag;             // [2]  NaN criteria, dt_min clamps
@@ -55,8 +57,9 @@ struct gd_ctx {
     double t_pred;
     int64_t block_steps, particle_steps, launches;
     int last_force_kernel;
-    int ipar_variant, ipar_split;        // tuning overrides (-1 / 0 = automatic)
-    int js_bi, js_cluster, js_ctas_per_sm;
+    int64_t ipar_small_max_nact;         // js_hi < n_act <= this: i-parallel kernel with 32-sink tiles
+    int grid_s, grid_l, js_clusters;     // launch shapes (gdk_force_setup)
+    int *h_geom_s, *h_geom_l;            // host copies of the geometry tables ({splits, units per split} pairs)
     int last_geom[4];                    // geometry of the last force launch: variant, i-tiles (or groups), splits, units per split
     unsigned int epoch, ticket_min_base, ticket_cmp_base;
     int sm_count;
@@ -85,6 +88,8 @@ int gdk_pack_sources(gd_ctx *c, const double *m, const double *x, const double *
 int gdk_iota(gd_ctx *c, int32_t *idx, int64_t n);
 
 int gdk_force(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out);   // gd_force.cu
+int gdk_force_dev(gd_ctx *c);
+int gdk_force_setup(gd_ctx *c);
 
 int gdk_correct(gd_ctx *c, double t_next);                                                   // gd_correct.cu
 int gdk_next_block(gd_ctx *c);                                                               // gd_next_block.cu
