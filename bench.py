@@ -217,7 +217,7 @@ def main_ours(args):
         torch.cuda.synchronize()
 
     for _ in range(args.warmup):
-        run_step(gd, m_d, x_d, v_d, w, t_end, host=False, profile=True)
+        run_step(gd, m_d, x_d, v_d, w, t_end, host=False, profile=False)
     run_step(gd, m_h, x_h, v_h, w, t_end, host=True, profile=False)
 
     # ---- timed region: K steps, inputs resident in HBM, L2 flushed between steps ----
@@ -228,9 +228,14 @@ def main_ours(args):
         e0.record()
         for _ in range(args.steps):
             flush_l2(torch, l2buf)
-            results.append(run_step(gd, m_d, x_d, v_d, w, t_end, host=False, profile=True))
+            results.append(run_step(gd, m_d, x_d, v_d, w, t_end, host=False, profile=False))
         e1.record()
         barrier()
+        # The timed steps replay the captured block-step graph, in which a single launch cannot be bracketed by
+        # events.  The per-launch durations of the force kernels come from one more pass of the SAME step, still
+        # under the clock sampler, taken through the explicit call sequence with the library's event timing on.
+        flush_l2(torch, l2buf)
+        prof_pass = run_step(gd, m_d, x_d, v_d, w, t_end, host=False, profile=True)
     sec = e0.elapsed_time(e1) * 1e-3
     # ---- end to end: K steps through host buffers (H2D of inputs and D2H of the state inside) ----
     e2e_results = []
@@ -253,7 +258,7 @@ def main_ours(args):
             dist.destroy_process_group()
         return
     return finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, sec_e2e, pairs, pairs_e2e,
-                       clocks.summary())
+                       clocks.summary(), prof_pass)
 
 
 # dram bytes per launch of the dominant force kernel from the committed `ncu --set full` capture under profiles/
@@ -261,22 +266,26 @@ def main_ours(args):
 NCU_TRAFFIC_BYTES = {}
 
 
-def finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, sec_e2e, pairs, pairs_e2e, clocks):
+def finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, sec_e2e, pairs, pairs_e2e, clocks,
+                prof_pass):
     K = args.steps
-    prof = {k: {f: sum(r["prof"][k][f] for r in results) for f in ("launches", "ms", "pairs")} for k in ("ipar", "jsplit")}
+    prof = {k: {f: prof_pass["prof"][k][f] for f in ("launches", "ms", "pairs")}
+            for k in ("ipar", "jsplit", "ipar_small")}
     dom = max(prof, key=lambda k: prof[k]["ms"])
     d = prof[dom]
     achieved = FLOP_PER_PAIR * d["pairs"] / (d["ms"] * 1e-3) / 1e12 if d["ms"] > 0 else 0.0
     peak_probe, _ = gd.fp64_peak_probe(1 << 16)
     roofline = {
-        "bound": "alu", "kernel": {"ipar": "k_force_ipar", "jsplit": "k_force_jsplit"}[dom],
+        "bound": "alu", "kernel": {"ipar": "k_force_ipar<2,1>", "jsplit": "k_force_jsplit", "ipar_small": "k_force_ipar<1,4>"}[dom],
         "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
         "traffic": NCU_TRAFFIC_BYTES.get((args.workload, dom)),
         "peak_source": "derived: 148 SM x 64 DFMA lanes/clk x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
                        "entry); register-only DFMA probe on this box: %.2f TFLOP/s" % (peak_probe / 1e12),
         "launches": int(d["launches"]), "avg_launch_us": 1e3 * d["ms"] / max(d["launches"], 1),
         "flop_per_launch": FLOP_PER_PAIR * d["pairs"] / max(d["launches"], 1),
-        "share_of_step": d["ms"] * 1e-3 / sec,
+        "share_of_step": d["ms"] * 1e-3 / (sec / K),
+        "timing": "per-launch CUDA events (library stream) over one extra pass of the same step through the explicit "
+                  "call sequence; the timed steps replay a captured graph",
         "by_kernel": {k: {"launches": int(v["launches"]), "ms": v["ms"],
                           "tflops60": (FLOP_PER_PAIR * v["pairs"] / (v["ms"] * 1e-3) / 1e12) if v["ms"] > 0 else 0.0}
                       for k, v in prof.items()},

@@ -101,6 +101,7 @@ static size_t gd_carve(gd_dev *d, void *base, int64_t np, int64_t pcap)
     t.blockmin = w.take<double>(GD_SCAN_MAX_BLOCKS);
     t.agg = w.take<unsigned long long>(GD_SCAN_MAX_BLOCKS);
     t.ticket = w.take<unsigned int>(4);
+    t.ctrl = w.take<gd_ctrl>(1);
     t.tile_ticket = w.take<unsigned int>(np / 32);
     t.work = w.take<unsigned int>(4);
     t.geom_s = w.take<int2>(np / 32 + 2);
@@ -130,6 +131,8 @@ extern "C" void gd_destroy(gd_ctx *ctx)
 {
     if (!ctx) return;
     if (ctx->h_cell) cudaFreeHost(ctx->h_cell);
+    if (ctx->h_ctrl) cudaFreeHost(ctx->h_ctrl);
+    if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);
     free(ctx->h_geom_s);
     free(ctx->h_geom_l);
     if (ctx->ev_created)
@@ -159,6 +162,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->dt_max = ldexp(1.0, -GD_LEVEL_MIN);
     c->dt_min = ldexp(1.0, -GD_LEVEL_MAX);
     c->halving_mode = 1;
+    c->use_graph = 1;
     c->jsplit_max_nact = 512;
     c->ipar_small_max_nact = 2048;
     c->stream = (cudaStream_t)stream;
@@ -167,6 +171,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (e == cudaSuccess) e = cudaHostAlloc((void **)&c->h_cell, 64, cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaHostAlloc((void **)&c->h_ctrl, 2 * sizeof(gd_ctrl), cudaHostAllocDefault);
     if (e != cudaSuccess) {
         gd_fail_cuda(nullptr, e, "gd_init: no usable CUDA device (there is no CPU fallback)");
         free(c);
@@ -181,8 +186,6 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
 static int gd_prepare(gd_ctx *c)
 {
     GD_CUDA(c, cudaMemsetAsync(c->d.blockmin, 0, (char *)c->d.phi - (char *)c->d.blockmin, c->stream));
-    c->epoch = 0;
-    c->ticket_min_base = c->ticket_cmp_base = 0;
     return gdk_force_setup(c);
 }
 
@@ -229,17 +232,24 @@ extern "C" int gd_init_host(gd_ctx **out, int64_t n, const double *m_host, const
     return rc;
 }
 
+// the captured graph froze the kernel arguments: options that change them invalidate it
+static void gd_graph_drop(gd_ctx *c)
+{
+    if (c->step_graph) { cudaGraphExecDestroy(c->step_graph); c->step_graph = nullptr; }
+}
+
 extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
 {
     if (!c || !key) return GD_EINVAL;
-    if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; return GD_OK; }
-    if (!strcmp(key, "ipar_small_max_nact")) { c->ipar_small_max_nact = (int64_t)value; return GD_OK; }
+    if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
+    if (!strcmp(key, "ipar_small_max_nact")) { c->ipar_small_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
+    if (!strcmp(key, "use_graph")) { c->use_graph = value != 0.0; return GD_OK; }
     if (!strcmp(key, "profile")) {
         int rc = gd_prof_drain(c);
         c->profile = (int)value;
         return rc;
     }
-    if (!strcmp(key, "halving_mode")) { c->halving_mode = value != 0.0; return GD_OK; }
+    if (!strcmp(key, "halving_mode")) { c->halving_mode = value != 0.0; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "dt_level_min") || !strcmp(key, "dt_level_max")) {
         int lv = (int)value;
         if (lv < 0 || lv > 52) return gd_fail(c, GD_EINVAL, "gd_set_option: level out of range");
@@ -250,6 +260,7 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
         if (lo > hi) return GD_OK;                 // transient while the caller sets both; checked below once ordered
         c->dt_max = ldexp(1.0, -lo);
         c->dt_min = ldexp(1.0, -hi);
+        gd_graph_drop(c);
         // the initial steps depend on the limits: redo them from the stored a, jerk
         int rc = gdk_unpack_state(c, nullptr, nullptr, c->d.a1, c->d.j1, nullptr, nullptr);
         if (!rc) rc = gdk_initial_dt(c);
@@ -347,9 +358,78 @@ static int gd_one_step(gd_ctx *c)
     return rc;
 }
 
+// ---- the block-step graph -----------------------------------------------------------------------
+// GD_GRAPH_STEPS block steps -- next_block, predict, the three force kernels (the device picks one), correct --
+// are captured once from an internal stream with every launch shape independent of n_act, and replayed on the
+// context's stream.  The host only uploads the limits (gd_ctrl) and reads the counters back once per burst of
+// replays; steps enqueued past the end of the run find `finished` set and do nothing.
+#define GD_GRAPH_STEPS 32
+
+static int gd_graph_build(gd_ctx *c)
+{
+    cudaStream_t cap = nullptr, user = c->stream;
+    GD_CUDA(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    const int64_t launches_before = c->launches;
+    c->stream = cap;
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeRelaxed);
+    int rc = 0;
+    if (e == cudaSuccess) {
+        for (int k = 0; k < GD_GRAPH_STEPS && !rc; ++k) {
+            rc = gdk_next_block(c, true);
+            if (!rc) rc = gdk_predict(c, 0.0, true);
+            if (!rc) rc = gdk_force_dev(c);
+            if (!rc) rc = gdk_correct(c, 0.0, true);
+        }
+        cudaGraph_t g = nullptr;
+        e = cudaStreamEndCapture(cap, &g);
+        if (e == cudaSuccess && !rc) e = cudaGraphInstantiate(&c->step_graph, g, 0);
+        if (g) cudaGraphDestroy(g);
+    }
+    c->stream = user;
+    c->graph_nodes = c->launches - launches_before;
+    c->launches = launches_before;
+    cudaStreamDestroy(cap);
+    if (rc) return rc;
+    if (e != cudaSuccess) return gd_fail_cuda(c, e, "gd_graph_build");
+    return GD_OK;
+}
+
+static int gd_run_graph(gd_ctx *c, double t_end, int64_t max_steps, int64_t *steps_out, int64_t *psteps_out)
+{
+    if (!c->step_graph) {
+        int rc = gd_graph_build(c);
+        if (rc) return rc;
+    }
+    gd_ctrl *up = c->h_ctrl, *down = c->h_ctrl + 1;
+    up->t_end = t_end;
+    up->t = c->t;
+    up->max_steps = max_steps;
+    up->steps = up->psteps = up->finished = 0;
+    GD_CUDA(c, cudaMemcpyAsync(c->d.ctrl, up, sizeof(gd_ctrl), cudaMemcpyHostToDevice, c->stream));
+    int burst = 1;
+    for (;;) {
+        for (int b = 0; b < burst; ++b) GD_CUDA(c, cudaGraphLaunch(c->step_graph, c->stream));
+        c->launches += (int64_t)burst * c->graph_nodes;
+        GD_CUDA(c, cudaMemcpyAsync(down, c->d.ctrl, sizeof(gd_ctrl), cudaMemcpyDeviceToHost, c->stream));
+        GD_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (down->finished) break;
+        if (burst < 4) burst *= 2;
+    }
+    c->t = down->t;
+    c->block_steps += down->steps;
+    c->particle_steps += down->psteps;
+    c->have_block = c->have_force = c->have_pred = false;
+    if (steps_out) *steps_out = down->steps;
+    if (psteps_out) *psteps_out = down->psteps;
+    return GD_OK;
+}
+
 extern "C" int gd_step(gd_ctx *c, int64_t n_steps, int64_t *particle_steps_host)
 {
     if (!c) return GD_EINVAL;
+    if (c->lvl_min > c->lvl_max) return gd_fail(c, GD_ESTATE, "gd_step: dt_level_min > dt_level_max");
+    if (c->use_graph && !c->profile && n_steps >= GD_GRAPH_STEPS / 2)
+        return gd_run_graph(c, INFINITY, n_steps, nullptr, particle_steps_host);
     int64_t before = c->particle_steps;
     for (int64_t s = 0; s < n_steps; ++s) {
         int rc = gd_one_step(c);
@@ -363,6 +443,10 @@ extern "C" int gd_step(gd_ctx *c, int64_t n_steps, int64_t *particle_steps_host)
 extern "C" int gd_run_until(gd_ctx *c, double t_end, int64_t max_steps, int64_t *steps_host, int64_t *particle_steps_host)
 {
     if (!c) return GD_EINVAL;
+    if (t_end != t_end) return gd_fail(c, GD_EINVAL, "gd_run_until: t_end is NaN");
+    if (c->lvl_min > c->lvl_max) return gd_fail(c, GD_ESTATE, "gd_run_until: dt_level_min > dt_level_max");
+    if (c->use_graph && !c->profile && c->t < t_end && max_steps != 0)
+        return gd_run_graph(c, t_end, max_steps, steps_host, particle_steps_host);
     int64_t before = c->particle_steps, steps = 0;
     while (c->t < t_end && (max_steps < 0 || steps < max_steps)) {
         int rc = gd_one_step(c);

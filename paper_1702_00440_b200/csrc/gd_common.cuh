@@ -15,6 +15,16 @@
 #define GD_TILE_J 256            // sources per shared-memory stage of the force kernels; np is a multiple
 #define GD_UNIT_J 64             // granularity of a CTA's source range (TMA copies stay 16-byte aligned)
 
+// Device-resident run control of the captured block-step graph (gd_step / gd_run_until): the host writes the
+// limits, the kernels keep the counters, and once `finished` is set every later kernel of the graph does nothing.
+struct gd_ctrl {
+    double t_end;                // stop once t >= t_end
+    double t;                    // time reached (k_correct_timestep)
+    long long max_steps;         // stop after this many block steps of the current run (< 0: no limit)
+    long long steps, psteps;     // block steps / particle steps taken in the current run
+    long long finished;          // set by k_block_min
+};
+
 struct gd_dev {
     double4 *xm, *vt, *ad, *jk;
     double *tnext;
@@ -25,7 +35,8 @@ struct gd_dev {
     double *partial;             // [pcap,6] partial sums of split force evaluations
     double *blockmin;            // [GD_SCAN_MAX_BLOCKS] per-block minima of tnext
     unsigned long long *agg;     // [GD_SCAN_MAX_BLOCKS] {epoch:32 | count:32} per-block aggregates of the compaction
-    unsigned int *ticket;        // [4] monotonically increasing block tickets (never reset)
+    unsigned int *ticket;        // [4] {k_block_min arrivals, k_block_compact block numbers, scan epoch, -}: re-armed by the last block
+    gd_ctrl *ctrl;
     unsigned int *tile_ticket;   // [np / 32] arrivals per i-tile of a split force evaluation (re-armed to 0 by the last CTA)
     unsigned int *work;          // [4] {next unit ticket, CTAs finished} of the persistent force grid (re-armed by the last CTA)
     int2 *geom_s, *geom_l;       // [np / 32 + 2], [np / 256 + 2]: i-tiles -> {source splits, units per split}
@@ -61,7 +72,10 @@ struct gd_ctx {
     int grid_s, grid_l, js_clusters;     // launch shapes (gdk_force_setup)
     int *h_geom_s, *h_geom_l;            // host copies of the geometry tables ({splits, units per split} pairs)
     int last_geom[4];                    // geometry of the last force launch: variant, i-tiles (or groups), splits, units per split
-    unsigned int epoch, ticket_min_base, ticket_cmp_base;
+    cudaGraphExec_t step_graph;          // GD_GRAPH_STEPS block steps captured from the stream (built on first use)
+    gd_ctrl *h_ctrl;                     // pinned host mirror of d.ctrl
+    int use_graph;
+    int64_t graph_nodes;                 // kernel nodes in step_graph
     int sm_count;
     // optional CUDA-event timing of the force launches ("profile" option; see gd_get_profile)
     int profile;
@@ -80,7 +94,7 @@ int gd_prof_drain(gd_ctx *c);
 
 // ---- launch wrappers (one per kernel file); all enqueue on c->stream and bump c->launches -------------
 int gdk_pack_state(gd_ctx *c, const double *m, const double *x, const double *v);           // gd_predict.cu
-int gdk_predict(gd_ctx *c, double t);
+int gdk_predict(gd_ctx *c, double t, bool dev = false);
 int gdk_initial_dt(gd_ctx *c);
 int gdk_unpack_state(gd_ctx *c, double *x, double *v, double *a, double *j, double *t, double *dt);
 int gdk_unpack_predicted(gd_ctx *c, double *xp, double *vp);
@@ -91,8 +105,8 @@ int gdk_force(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, doubl
 int gdk_force_dev(gd_ctx *c);
 int gdk_force_setup(gd_ctx *c);
 
-int gdk_correct(gd_ctx *c, double t_next);                                                   // gd_correct.cu
-int gdk_next_block(gd_ctx *c);                                                               // gd_next_block.cu
+int gdk_correct(gd_ctx *c, double t_next, bool dev = false);                                 // gd_correct.cu
+int gdk_next_block(gd_ctx *c, bool dev = false);                                             // gd_next_block.cu
 int gdk_energy(gd_ctx *c);                                                                   // gd_energy.cu
 int gdk_fp64_probe(int iters, double *flops, double *ms);                                    // gd_probe.cu
 

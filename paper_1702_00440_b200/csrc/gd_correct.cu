@@ -37,16 +37,22 @@ __device__ __forceinline__ gd_corr1 gd_correct_component(double xp, double vp, d
 }
 
 __global__ void __launch_bounds__(GD_CB)
-k_correct_timestep(gd_dev d, int n_act, double t_next, double eta, double dt_min, double dt_max, int halving_mode, int lvl_cap)
+k_correct_timestep(gd_dev d, int n_act, double t_next, double eta, double dt_min, double dt_max, int halving_mode, int dev)
 {
+    // dev != 0 (block-step graph): the active count and t_next come from device memory, the grid is fixed and
+    // strides over the list, and block 0 advances the run counters once the step is committed
+    if (dev) {
+        if (d.ctrl->finished) return;
+        n_act = (int)((const long long *)d.cell)[1];
+        t_next = d.cell[0];
+    }
     __shared__ unsigned int s_hist[64];
     __shared__ unsigned int s_diag[2];
     if (threadIdx.x < 64) s_hist[threadIdx.x] = 0;
     if (threadIdx.x < 2) s_diag[threadIdx.x] = 0;
     __syncthreads();
 
-    int k = blockIdx.x * GD_CB + threadIdx.x;
-    if (k < n_act) {
+    for (int k = blockIdx.x * GD_CB + threadIdx.x; k < n_act; k += gridDim.x * GD_CB) {
         const int32_t i = d.idx[k];
         double2 pxy = d.pxy[i], pzm = d.pzm[i], pvxy = d.vxy[i];
         double pvz = d.vz[i];
@@ -96,14 +102,22 @@ k_correct_timestep(gd_dev d, int n_act, double t_next, double eta, double dt_min
     __syncthreads();
     if (threadIdx.x < 64 && s_hist[threadIdx.x]) atomicAdd((unsigned long long *)&d.hist[threadIdx.x], (unsigned long long)s_hist[threadIdx.x]);
     if (threadIdx.x < 2 && s_diag[threadIdx.x]) atomicAdd((unsigned long long *)&d.diag[threadIdx.x], (unsigned long long)s_diag[threadIdx.x]);
+    if (dev && blockIdx.x == 0 && threadIdx.x == 0) {
+        gd_ctrl *ct = d.ctrl;
+        ct->t = t_next;
+        ct->steps += 1;
+        ct->psteps += n_act;
+    }
 }
 
-int gdk_correct(gd_ctx *c, double t_next)
+int gdk_correct(gd_ctx *c, double t_next, bool dev)
 {
-    if (c->n_act <= 0) return 0;
-    unsigned blocks = (unsigned)((c->n_act + GD_CB - 1) / GD_CB);
-    k_correct_timestep<<<blocks, GD_CB, 0, c->stream>>>(c->d, (int)c->n_act, t_next, c->eta, c->dt_min, c->dt_max,
-                                                        c->halving_mode, c->lvl_max);
+    if (!dev && c->n_act <= 0) return 0;
+    const int64_t want = dev ? c->n : c->n_act;
+    int64_t blocks = (want + GD_CB - 1) / GD_CB;
+    if (dev && blocks > 4 * (int64_t)c->sm_count) blocks = 4 * (int64_t)c->sm_count;
+    k_correct_timestep<<<(unsigned)blocks, GD_CB, 0, c->stream>>>(c->d, (int)c->n_act, t_next, c->eta, c->dt_min, c->dt_max,
+                                                                  c->halving_mode, dev ? 1 : 0);
     GD_LAUNCH_CHECK(c, "k_correct_timestep");
     return 0;
 }

@@ -29,6 +29,7 @@ namespace cg = cooperative_groups;
 #define GD_JS_THREADS 256
 #define GD_JS_WARPS (GD_JS_THREADS / 32)
 #define GD_JS_CLUSTER 8
+#define GD_JS_MAX_CPT 16          // clusters per i-tile: more only lengthens the fold
 
 // ---------------------------------------------------------------------------------------------------------
 // q = s^(-1/2): MUFU.RSQ64H seed (relative error ~2^-21: it sees the upper 32 bits of s only) followed by one
@@ -370,7 +371,7 @@ k_force_jsplit(gd_dev d, gd_fargs fa)
     const int n_clusters = gridDim.x / cdim;
     const int i_tiles = (n_act + 31) / 32;                         // <= n_clusters (the host bounds hi)
     int cpt = n_clusters / i_tiles;                                // clusters per i-tile
-    cpt = max(1, min(cpt, fa.n_units / cdim));                     // at least one unit per CTA where the sources allow it
+    cpt = max(1, min(min(cpt, GD_JS_MAX_CPT), fa.n_units / cdim)); // at least one unit per CTA where the sources allow it; bounded fold
     const int c = blockIdx.x / cdim;
     const int i_tile = c / cpt, part = c - i_tile * cpt;
     if (i_tile >= i_tiles) return;                                 // whole clusters leave together

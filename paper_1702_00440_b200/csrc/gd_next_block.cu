@@ -2,12 +2,16 @@
 //   t_next = min_i (t_i + dt_i) ;  active = { i ascending : t_i + dt_i == t_next }
 // Times are exact dyadic doubles, so the comparison is exact and the result is unique (R13, R20).
 //
-// Two kernels, both bandwidth/latency bound at 8 B per particle each:
+// Large systems: two kernels, both bandwidth/latency bound at 8 B per particle each (small systems: the
+// single-CTA k_block_select below):
 //   k_block_min      grid-wide minimum of tnext[]; the last block to finish (ticket) folds the per-block minima
 //   k_block_compact  stream compaction by warp ballot + prefix sums: each block counts its flags, publishes
 //                    the count, sums the counts of all lower-numbered blocks, and writes its indices in order.
-// Block numbers are handed out by an atomic ticket, so a block only ever waits for blocks that already run;
-// tickets and aggregates carry the launch epoch and are never reset.
+// Block numbers are handed out by an atomic ticket, so a block only ever waits for blocks that already run.
+// Tickets are re-armed by the last block to take one; aggregates carry a launch epoch that k_block_min advances
+// in device memory, so that both kernels can be replayed from a captured graph with frozen arguments.
+// dev != 0 (block-step graph): k_block_min also decides whether the run is over (gd_ctrl) and, if it is, marks it
+// finished and publishes an empty active list; every later kernel of the graph then does nothing.
 #include "gd_common.cuh"
 #include <stdio.h>
 
@@ -19,8 +23,9 @@ __device__ __forceinline__ double gd_warp_min(double v)
 }
 
 __global__ void __launch_bounds__(GD_SCAN_THREADS)
-k_block_min(gd_dev d, int64_t np, int per_block, unsigned int ticket_base)
+k_block_min(gd_dev d, int64_t np, int per_block, int dev)
 {
+    if (dev && d.ctrl->finished) return;
     __shared__ double s_min[GD_SCAN_THREADS / 32];
     __shared__ bool s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -37,8 +42,9 @@ k_block_min(gd_dev d, int64_t np, int per_block, unsigned int ticket_base)
         if (lane == 0) {
             d.blockmin[blockIdx.x] = m;
             __threadfence();
-            unsigned int tk = atomicAdd(&d.ticket[0], 1u) - ticket_base;
+            unsigned int tk = atomicAdd(&d.ticket[0], 1u);
             s_last = (tk == gridDim.x - 1);
+            if (s_last) d.ticket[0] = 0u;                        // every block has arrived: re-arm
         }
     }
     __syncthreads();
@@ -51,23 +57,38 @@ k_block_min(gd_dev d, int64_t np, int per_block, unsigned int ticket_base)
         __syncthreads();
         if (warp == 0) {
             m = gd_warp_min(s_min[lane]);
-            if (lane == 0) d.cell[0] = m;
+            if (lane == 0) {
+                unsigned int ep = d.ticket[2] + 1u;
+                d.ticket[2] = ep ? ep : 1u;                      // epoch of this scan; 0 = freshly cleared scratch
+                gd_ctrl *ct = d.ctrl;
+                if (dev && (ct->t >= ct->t_end || (ct->max_steps >= 0 && ct->steps >= ct->max_steps))) {
+                    ct->finished = 1;
+                    ((long long *)d.cell)[1] = 0;                // empty active list: the force and corrector kernels fall through
+                } else {
+                    d.cell[0] = m;
+                }
+            }
         }
     }
 }
 
 // per_block <= 32 * GD_SCAN_THREADS: every thread keeps its flags in one 32-bit mask
 __global__ void __launch_bounds__(GD_SCAN_THREADS)
-k_block_compact(gd_dev d, int64_t np, int per_block, unsigned int ticket_base, unsigned int epoch)
+k_block_compact(gd_dev d, int64_t np, int per_block, int dev)
 {
+    if (dev && d.ctrl->finished) return;
     __shared__ unsigned int s_bid;
     __shared__ int s_warp[GD_SCAN_THREADS / 32];
     __shared__ int s_round_base[33];
     __shared__ int s_prefix;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_bid = atomicAdd(&d.ticket[1], 1u) - ticket_base;
+    if (tid == 0) {
+        s_bid = atomicAdd(&d.ticket[1], 1u);
+        if (s_bid == gridDim.x - 1) d.ticket[1] = 0u;            // every block has its number: re-arm
+    }
     __syncthreads();
     const unsigned int bid = s_bid;
+    const unsigned int epoch = d.ticket[2];
     const double t_next = d.cell[0];
     const int64_t begin = (int64_t)bid * per_block;
     const int64_t end = min(np, begin + per_block);
@@ -138,8 +159,88 @@ k_block_compact(gd_dev d, int64_t np, int per_block, unsigned int ticket_base, u
     if (bid == gridDim.x - 1 && tid == 0) ((long long *)d.cell)[1] = (long long)(prefix + total);
 }
 
-int gdk_next_block(gd_ctx *c)
+// ---------------------------------------------------------------------------------------------------------
+// Small systems (np <= 1024 * 64): one CTA does both passes -- no tickets, no fences, one launch.  Thread t owns the
+// contiguous chunk [t * R, (t + 1) * R) of tnext (vector loads of whole lines), so the ascending order of the
+// active list is the thread order: block minimum, per-thread match counts, one block-wide exclusive scan, ordered
+// writes.  KEEP holds the chunk in registers between the passes; otherwise the second pass re-reads it from L2.
+template <int R, bool KEEP>
+__global__ void __launch_bounds__(GD_SCAN_THREADS)
+k_block_select(gd_dev d, int64_t np, int dev)
 {
+    __shared__ double s_min[32];
+    __shared__ int s_cnt[32];
+    if (dev && d.ctrl->finished) return;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t base = (int64_t)tid * R;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    double v[KEEP ? R : 1];
+    double m = inf;
+#pragma unroll
+    for (int k = 0; k < R; k += 2) {
+        double2 x = (base + k < np) ? __ldcg(reinterpret_cast<const double2 *>(d.tnext + base + k)) : make_double2(inf, inf);
+        if (KEEP) { v[k] = x.x; v[k + 1] = x.y; }
+        m = fmin(m, fmin(x.x, x.y));
+    }
+    m = gd_warp_min(m);
+    if (lane == 0) s_min[warp] = m;
+    __syncthreads();
+    m = gd_warp_min(s_min[lane]);                                // every warp folds the 32 warp minima itself
+
+    unsigned long long mask = 0ull;                              // R <= 64 match flags of this thread's chunk
+#pragma unroll
+    for (int k = 0; k < R; k += 2) {
+        double2 x;
+        if (KEEP) x = make_double2(v[k], v[k + 1]);
+        else x = (base + k < np) ? __ldcg(reinterpret_cast<const double2 *>(d.tnext + base + k)) : make_double2(inf, inf);
+        mask |= (unsigned long long)(x.x == m) << k;
+        mask |= (unsigned long long)(x.y == m) << (k + 1);
+    }
+    const int cnt = __popcll(mask);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += u; }
+    if (lane == 31) s_cnt[warp] = incl;
+    __syncthreads();
+    int wsum = s_cnt[lane], wincl = wsum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, wincl, o); if (lane >= o) wincl += u; }
+    const int total = __shfl_sync(0xffffffffu, wincl, 31);
+    int pos = __shfl_sync(0xffffffffu, wincl - wsum, warp) + incl - cnt;     // exclusive prefix of this thread
+
+    bool stop = false;
+    if (dev) {
+        const gd_ctrl *ct = d.ctrl;
+        stop = ct->t >= ct->t_end || (ct->max_steps >= 0 && ct->steps >= ct->max_steps);
+    }
+    if (!stop) {
+        while (mask) {
+            int k = __ffsll((long long)mask) - 1;
+            mask &= mask - 1;
+            d.idx[pos++] = (int32_t)(base + k);
+        }
+    }
+    if (tid == 0) {
+        if (stop) {
+            d.ctrl->finished = 1;
+            ((long long *)d.cell)[1] = 0;
+        } else {
+            d.cell[0] = m;
+            ((long long *)d.cell)[1] = (long long)total;
+        }
+    }
+}
+
+int gdk_next_block(gd_ctx *c, bool dev)
+{
+    if (c->np <= 64 * GD_SCAN_THREADS) {
+        const int dv = dev ? 1 : 0;
+        if (c->np <= 4 * GD_SCAN_THREADS) k_block_select<4, true><<<1, GD_SCAN_THREADS, 0, c->stream>>>(c->d, c->np, dv);
+        else if (c->np <= 16 * GD_SCAN_THREADS) k_block_select<16, true><<<1, GD_SCAN_THREADS, 0, c->stream>>>(c->d, c->np, dv);
+        else k_block_select<64, false><<<1, GD_SCAN_THREADS, 0, c->stream>>>(c->d, c->np, dv);
+        GD_LAUNCH_CHECK(c, "k_block_select");
+        return 0;
+    }
     // contiguous ranges of whole 1024-element rounds; at most 32 rounds per block
     int64_t rounds_total = (c->np + GD_SCAN_THREADS - 1) / GD_SCAN_THREADS;
     int64_t blocks = rounds_total < 2 * c->sm_count ? rounds_total : 2 * c->sm_count;
@@ -156,13 +257,9 @@ int gdk_next_block(gd_ctx *c)
     blocks = (rounds_total + rounds_per_block - 1) / rounds_per_block;
     int per_block = (int)(rounds_per_block * GD_SCAN_THREADS);
 
-    k_block_min<<<(unsigned)blocks, GD_SCAN_THREADS, 0, c->stream>>>(c->d, c->np, per_block, c->ticket_min_base);
+    k_block_min<<<(unsigned)blocks, GD_SCAN_THREADS, 0, c->stream>>>(c->d, c->np, per_block, dev ? 1 : 0);
     GD_LAUNCH_CHECK(c, "k_block_min");
-    c->ticket_min_base += (unsigned int)blocks;
-    c->epoch += 1;
-    if (c->epoch == 0) c->epoch = 1;     // 0 is the value of freshly cleared scratch
-    k_block_compact<<<(unsigned)blocks, GD_SCAN_THREADS, 0, c->stream>>>(c->d, c->np, per_block, c->ticket_cmp_base, c->epoch);
+    k_block_compact<<<(unsigned)blocks, GD_SCAN_THREADS, 0, c->stream>>>(c->d, c->np, per_block, dev ? 1 : 0);
     GD_LAUNCH_CHECK(c, "k_block_compact");
-    c->ticket_cmp_base += (unsigned int)blocks;
     return 0;
 }

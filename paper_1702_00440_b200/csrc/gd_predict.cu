@@ -81,10 +81,15 @@ int gdk_iota(gd_ctx *c, int32_t *idx, int64_t n)
 //   D = t - t_i ;  xp = x + v D + a D^2/2 + jerk D^3/6 ;  vp = v + a D + jerk D^2/2
 // Every product and sum is rounded separately (no FMA contraction), left to right as written, so that the
 // predicted records are reproducible bit for bit by any IEEE implementation of the same expression.
-__global__ void __launch_bounds__(GD_PB) k_predict(gd_dev d, int64_t n, double t)
+// dev != 0 (block-step graph): t is the t_next that k_block_min left in device memory.
+__global__ void __launch_bounds__(GD_PB) k_predict(gd_dev d, int64_t n, double t, int dev)
 {
     int64_t i = (int64_t)blockIdx.x * GD_PB + threadIdx.x;
     if (i >= n) return;
+    if (dev) {
+        if (d.ctrl->finished) return;
+        t = d.cell[0];
+    }
     double4 xm = d.xm[i], vt = d.vt[i], ad = d.ad[i], jk = d.jk[i];
     double D = __dsub_rn(t, vt.w);
     double DD = __dmul_rn(D, D);
@@ -103,9 +108,9 @@ __global__ void __launch_bounds__(GD_PB) k_predict(gd_dev d, int64_t n, double t
     d.vz[i] = vzp;
 }
 
-int gdk_predict(gd_ctx *c, double t)
+int gdk_predict(gd_ctx *c, double t, bool dev)
 {
-    k_predict<<<gd_blocks(c->n, GD_PB), GD_PB, 0, c->stream>>>(c->d, c->n, t);
+    k_predict<<<gd_blocks(c->n, GD_PB), GD_PB, 0, c->stream>>>(c->d, c->n, t, dev ? 1 : 0);
     GD_LAUNCH_CHECK(c, "k_predict");
     return 0;
 }

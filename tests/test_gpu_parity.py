@@ -166,12 +166,14 @@ def test_corrector_bit_exact_given_same_inputs(gd):
 
 
 # ----------------------------------------------------------------------------------------- active sets
-def test_next_block_against_oracle_on_synthetic_times(gd):
-    # drive the compaction with many different patterns by stepping a small system; every list must be the
-    # ascending exact-equality set of the oracle's definition applied to the GPU's own t, dt
-    w = W.config(1, n=3000)
+@pytest.mark.parametrize("n,steps", [(3000, 30), (10000, 12), (40000, 8), (70000, 6)])
+def test_next_block_against_oracle_on_synthetic_times(gd, n, steps):
+    # drive the compaction with many different patterns by stepping a system; every list must be the ascending
+    # exact-equality set of the oracle's definition applied to the GPU's own t, dt.  The sizes cover the three
+    # single-CTA variants (chunks of 4, 16, 64 per thread) and the two-kernel path for large systems.
+    w = W.config(1, n=n)
     h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
-    for _ in range(30):
+    for _ in range(steps):
         s = h.state(("t", "dt"))
         t_ref, act_ref = oracle.next_block(cpu(s["t"]), cpu(s["dt"]))
         t_next, n_act = h.next_block()
@@ -294,3 +296,40 @@ def test_host_init_equals_device_init(gd):
         assert np.array_equal(s1[k], s2[k]), k
     h1.close()
     h2.close()
+
+
+# ------------------------------------------------------------------------------ the captured block-step graph
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (4, 3000), (5, 2047)])
+def test_graph_replay_equals_explicit_calls(gd, cfg, n):
+    # gd_run_until / gd_step replay a captured graph whose kernels read n_act and t_next from device memory;
+    # the explicit call sequence passes them from the host.  Same kernels, same arithmetic: identical bits.
+    w = W.config(cfg, n=n)
+    hg = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    he = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    he.set_option("use_graph", 0)
+    for steps in (40, 70):                       # 70 is not a multiple of the graph's step count
+        pg = hg.step(steps)
+        pe = he.step(steps)
+        assert pg == pe and hg.t == he.t and hg.block_steps == he.block_steps == (40 if steps == 40 else 110)
+    sg, se = hg.state_host(), he.state_host()
+    for k in sg:
+        assert np.array_equal(sg[k], se[k]), k
+    hg.close(); he.close()
+
+
+def test_graph_run_until_matches_oracle_schedule(gd):
+    w = W.config(1)
+    t_end = 2.0 ** -5
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    steps, psteps = h.run_until(t_end)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    o.run(t_end)
+    assert h.t == o.t == t_end and steps == o.block_steps and psteps == o.particle_steps
+    hist, diag = h.level_histogram()
+    assert hist.sum() == psteps
+    s = h.state_host(("t", "dt"))
+    assert np.array_equal(s["t"], o.t_i) and np.array_equal(s["dt"], o.dt)
+    # a second call continues from where the first stopped; max_steps bounds it
+    steps2, _ = h.run_until(1.0, max_steps=5)
+    assert steps2 == 5 and h.block_steps == steps + 5
+    h.close()
