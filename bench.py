@@ -263,7 +263,7 @@ def main_ours(args):
 
 # dram bytes per launch of the dominant force kernel from the committed `ncu --set full` capture under profiles/
 # (None until one exists for the workload; see profiles/README.md)
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {("C2", "jsplit"): 938240, ("C2", "ipar"): 934656, ("C2", "ipar_small"): 936192}   # profiles/r1c_launches_graph_path.md
 
 
 def finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, sec_e2e, pairs, pairs_e2e, clocks,
