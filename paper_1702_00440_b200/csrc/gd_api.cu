@@ -106,12 +106,16 @@ static size_t gd_carve(gd_dev *d, void *base, int64_t np, int64_t pcap)
     t.work = w.take<unsigned int>(4);
     t.geom_s = w.take<int2>(np / 32 + 2);
     t.geom_l = w.take<int2>(np / 256 + 2);
+    t.lp_L = w.take<double>(256);
+    t.lp_cnt = w.take<int>(256);
+    t.lp_ctl = w.take<unsigned long long>(4);
     t.cell = w.take<double>(4);
     t.hist = w.take<long long>(64);
     t.diag = w.take<long long>(2);
     t.phi = w.take<double>(np);
     t.kin = w.take<double>(np);
     t.staging = w.take<double>(7 * np);
+    t.lp_rec = w.take<double4>(2 * (np + GD_LP_REC_SLACK));
     if (d) *d = t;
     return w.off;
 }
@@ -165,6 +169,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->use_graph = 1;
     c->jsplit_max_nact = 512;
     c->ipar_small_max_nact = 2048;
+    c->loop_max_nact = 512;
     c->stream = (cudaStream_t)stream;
     gd_carve(&c->d, ws, c->np, c->pcap);
     int dev = 0;
@@ -186,7 +191,9 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
 static int gd_prepare(gd_ctx *c)
 {
     GD_CUDA(c, cudaMemsetAsync(c->d.blockmin, 0, (char *)c->d.phi - (char *)c->d.blockmin, c->stream));
-    return gdk_force_setup(c);
+    int rc = gdk_force_setup(c);
+    if (!rc) rc = gdk_loop_setup(c);
+    return rc;
 }
 
 static int gd_init_common(gd_ctx *c, const double *m_dev, const double *x_dev, const double *v_dev)
@@ -244,6 +251,11 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
     if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "ipar_small_max_nact")) { c->ipar_small_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "use_graph")) { c->use_graph = value != 0.0; return GD_OK; }
+    if (!strcmp(key, "loop_max_nact")) {
+        c->loop_max_nact = (int64_t)value;
+        gd_graph_drop(c);
+        return gdk_loop_setup(c);
+    }
     if (!strcmp(key, "profile")) {
         int rc = gd_prof_drain(c);
         c->profile = (int)value;
@@ -375,7 +387,10 @@ static int gd_graph_build(gd_ctx *c)
     int rc = 0;
     if (e == cudaSuccess) {
         for (int k = 0; k < GD_GRAPH_STEPS && !rc; ++k) {
-            rc = gdk_next_block(c, true);
+            // the persistent loop takes every run of small steps; the stage kernels behind it take the one step
+            // that made it leave (active set above loop_hi) and do nothing once the run is finished
+            rc = gdk_loop(c);
+            if (!rc) rc = gdk_next_block(c, true);
             if (!rc) rc = gdk_predict(c, 0.0, true);
             if (!rc) rc = gdk_force_dev(c);
             if (!rc) rc = gdk_correct(c, 0.0, true);

@@ -46,9 +46,15 @@ struct gd_dev {
     double *phi;                 // [np] per-particle potential sums  (energy)
     double *kin;                 // [np] per-particle kinetic terms   (energy)
     void *staging;               // [7 np] doubles: staging for host<->device copies of m, x, v
+    // persistent block-step loop (gd_loop.cu)
+    double4 *lp_rec;             // [np + GD_LP_REC_SLACK][2] candidate records, one segment of S rows per CTA
+    double *lp_L;                // [256] smallest t_i + dt_i of every CTA's slice
+    int *lp_cnt;                 // [256] candidates per CTA
+    unsigned long long *lp_ctl;  // [4] {barrier arrivals, arrivals at the start of the current launch, particle steps in the loop, -}
 };
 
 #define GD_SCAN_MAX_BLOCKS 1024
+#define GD_LP_REC_SLACK (32 * 256)   // rows of lp_rec beyond np: slices are rounded up to 32 for up to 256 CTAs
 #define GD_PROF_POOL 64
 #define GD_SCAN_THREADS 1024
 
@@ -75,6 +81,9 @@ struct gd_ctx {
     cudaGraphExec_t step_graph;          // GD_GRAPH_STEPS block steps captured from the stream (built on first use)
     gd_ctrl *h_ctrl;                     // pinned host mirror of d.ctrl
     int use_graph;
+    int64_t loop_max_nact;               // option: largest active set the persistent loop takes (0 = loop off)
+    int loop_grid, loop_S, loop_hi;      // geometry of k_block_loop (loop_grid = 0: not usable)
+    size_t loop_smem;
     int64_t graph_nodes;                 // kernel nodes in step_graph
     int sm_count;
     // optional CUDA-event timing of the force launches ("profile" option; see gd_get_profile)
@@ -107,6 +116,8 @@ int gdk_force_setup(gd_ctx *c);
 
 int gdk_correct(gd_ctx *c, double t_next, bool dev = false);                                 // gd_correct.cu
 int gdk_next_block(gd_ctx *c, bool dev = false);                                             // gd_next_block.cu
+int gdk_loop_setup(gd_ctx *c);                                                               // gd_loop.cu
+int gdk_loop(gd_ctx *c);
 int gdk_energy(gd_ctx *c);                                                                   // gd_energy.cu
 int gdk_fp64_probe(int iters, double *flops, double *ms);                                    // gd_probe.cu
 

@@ -5,6 +5,7 @@
 // + 56 B written (pxy, pzm, vxy, vz) = 184 B.  Thread-per-particle, all accesses 16/32-byte vectors on
 // consecutive addresses (fully coalesced).
 #include "gd_common.cuh"
+#include "gd_hermite.cuh"
 
 #define GD_PB 256   // threads per block of the per-particle kernels
 
@@ -91,21 +92,11 @@ __global__ void __launch_bounds__(GD_PB) k_predict(gd_dev d, int64_t n, double t
         t = d.cell[0];
     }
     double4 xm = d.xm[i], vt = d.vt[i], ad = d.ad[i], jk = d.jk[i];
-    double D = __dsub_rn(t, vt.w);
-    double DD = __dmul_rn(D, D);
-    double D2 = __ddiv_rn(DD, 2.0);
-    double D3 = __ddiv_rn(__dmul_rn(DD, D), 6.0);
-#define GD_PX(x0, v0, a0, j0) \
-    __dadd_rn(__dadd_rn(__dadd_rn((x0), __dmul_rn((v0), D)), __dmul_rn((a0), D2)), __dmul_rn((j0), D3))
-#define GD_PV(v0, a0, j0) __dadd_rn(__dadd_rn((v0), __dmul_rn((a0), D)), __dmul_rn((j0), D2))
-    double xp = GD_PX(xm.x, vt.x, ad.x, jk.x), yp = GD_PX(xm.y, vt.y, ad.y, jk.y), zp = GD_PX(xm.z, vt.z, ad.z, jk.z);
-    double vxp = GD_PV(vt.x, ad.x, jk.x), vyp = GD_PV(vt.y, ad.y, jk.y), vzp = GD_PV(vt.z, ad.z, jk.z);
-#undef GD_PX
-#undef GD_PV
-    d.pxy[i] = make_double2(xp, yp);
-    d.pzm[i] = make_double2(zp, xm.w);
-    d.vxy[i] = make_double2(vxp, vyp);
-    d.vz[i] = vzp;
+    const gd_pred q = gd_predict_record(xm, vt, ad, jk, t);
+    d.pxy[i] = make_double2(q.x, q.y);
+    d.pzm[i] = make_double2(q.z, xm.w);
+    d.vxy[i] = make_double2(q.vx, q.vy);
+    d.vz[i] = q.vz;
 }
 
 int gdk_predict(gd_ctx *c, double t, bool dev)

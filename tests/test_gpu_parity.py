@@ -306,6 +306,7 @@ def test_graph_replay_equals_explicit_calls(gd, cfg, n):
     w = W.config(cfg, n=n)
     hg = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
     he = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    hg.set_option("loop_max_nact", 0)            # stage kernels only: the persistent loop sums in another order
     he.set_option("use_graph", 0)
     for steps in (40, 70):                       # 70 is not a multiple of the graph's step count
         pg = hg.step(steps)
@@ -333,3 +334,56 @@ def test_graph_run_until_matches_oracle_schedule(gd):
     steps2, _ = h.run_until(1.0, max_steps=5)
     assert steps2 == 5 and h.block_steps == steps + 5
     h.close()
+
+
+# ------------------------------------------------------------------------------ the persistent block-step loop
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (2, 16384), (3, 4096), (4, 6000), (5, 2047), (1, 100), (4, 40000)])
+def test_loop_first_100_block_steps_bit_exact_schedule(gd, cfg, n):
+    # gd_step through the graph whose first node is k_block_loop (small active sets are taken inside the persistent
+    # kernel, larger ones by the stage kernels behind it): the schedule must equal the oracle's bit for bit.
+    w = W.config(cfg, n=n)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    psteps = h.step(100)
+    for _ in range(100):
+        o.step()
+    assert h.t == o.t and h.block_steps == 100 and psteps == o.particle_steps
+    s = h.state_host(("x", "v", "a", "j", "t", "dt"))
+    assert np.array_equal(s["t"], o.t_i) and np.array_equal(s["dt"], o.dt)
+    assert np.abs(s["x"] - o.x).max() < 1e-12 and np.abs(s["v"] - o.v).max() < 1e-12
+    assert relnorm(s["a"], o.a).max() < 1e-12 and relnorm(s["j"], o.j).max() < 1e-12
+    hist, diag = h.level_histogram()
+    assert np.array_equal(hist, o.level_hist) and diag[0] == o.nan_count and diag[1] == o.dtmin_clamps
+    h.close()
+
+
+@pytest.mark.parametrize("hi", [1, 3, 8, 64, 1024])
+def test_loop_threshold_sweep_same_schedule(gd, hi):
+    # whatever share of the steps the loop takes (hi = largest active set it accepts), the schedule is the same
+    w = W.config(1)
+    t_end = 2.0 ** -5
+    ref = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    ref.set_option("loop_max_nact", 0)
+    ref.run_until(t_end)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h.set_option("loop_max_nact", hi)
+    steps, psteps = h.run_until(t_end)
+    assert h.t == ref.t == t_end and steps == ref.block_steps and psteps == ref.particle_steps
+    a, b = h.state_host(), ref.state_host()
+    assert np.array_equal(a["t"], b["t"]) and np.array_equal(a["dt"], b["dt"])
+    assert np.abs(a["x"] - b["x"]).max() < 1e-12
+    ha, _ = h.level_histogram(); hb, _ = ref.level_histogram()
+    assert np.array_equal(ha, hb)
+    h.close(); ref.close()
+
+
+def test_loop_is_run_to_run_identical(gd):
+    w = W.config(2, n=4096)
+    out = []
+    for _ in range(2):
+        h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+        h.step(200)
+        out.append(h.state_host())
+        h.close()
+    for k in out[0]:
+        assert np.array_equal(out[0][k], out[1][k]), k
