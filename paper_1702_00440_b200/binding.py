@@ -50,6 +50,7 @@ SYMBOLS = {
     "gd_get_active": (_int, [_vp, _vp, _i64]),
     "gd_get_level_histogram": (_int, [_vp, _vp, _vp]),
     "gd_get_profile": (_int, [_vp, _vp]),
+    "gd_get_loop_profile": (_int, [_vp, _vp]),
     "gd_fp64_peak_probe": (_int, [_int, _pdbl, _pdbl]),
 }
 
@@ -301,6 +302,12 @@ class Hermite:
         self._check(self._lib.gd_get_profile(self._h, p.ctypes.data))
         return {k: {"launches": int(p[4 * i]), "ms": float(p[4 * i + 1]), "pairs": float(p[4 * i + 2]),
                     "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit", "ipar_small"))}
+
+    def loop_profile(self) -> dict:
+        o = np.zeros(8, dtype=np.int64)
+        self._check(self._lib.gd_get_loop_profile(self._h, o.ctypes.data))
+        keys = ("particle_steps", "block_steps", "ns", "ns_force", "ns_barrier1", "ns_correct", "ns_barrier2", "launches")
+        return {k: int(v) for k, v in zip(keys, o)}
 
     def level_histogram(self) -> tuple[np.ndarray, np.ndarray]:
         h, d = np.zeros(64, dtype=np.int64), np.zeros(2, dtype=np.int64)

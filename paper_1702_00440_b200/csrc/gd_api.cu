@@ -67,7 +67,16 @@ void gd_prof_end(gd_ctx *c, int slot, int kind, double pairs)
 
 // ---- workspace -------------------------------------------------------------------------------------------
 static inline int64_t gd_pad(int64_t n) { return ((n + GD_TILE_J - 1) / GD_TILE_J) * GD_TILE_J; }
-static inline int64_t gd_pcap(int64_t np) { return (4 * np > (1 << 20)) ? 4 * np : (1 << 20); }
+// rows of 6 partial sums: the split force kernels need up to 4 np; the persistent loop (systems up to
+// GD_LP_MAX_NP particles) keeps one row per (CTA, active particle), for up to GD_LP_GRID_BOUND CTAs
+#define GD_LP_MAX_NP (1 << 19)
+#define GD_LP_GRID_BOUND 160
+static inline int64_t gd_pcap(int64_t np)
+{
+    int64_t r = (4 * np > (1 << 20)) ? 4 * np : (1 << 20);
+    if (np <= GD_LP_MAX_NP && GD_LP_GRID_BOUND * np > r) r = GD_LP_GRID_BOUND * np;
+    return r;
+}
 static inline size_t gd_up(size_t b) { return (b + 255) & ~(size_t)255; }
 
 struct gd_carver {
@@ -108,7 +117,7 @@ static size_t gd_carve(gd_dev *d, void *base, int64_t np, int64_t pcap)
     t.geom_l = w.take<int2>(np / 256 + 2);
     t.lp_L = w.take<double>(256);
     t.lp_cnt = w.take<int>(256);
-    t.lp_ctl = w.take<unsigned long long>(4);
+    t.lp_ctl = w.take<unsigned long long>(16);
     t.cell = w.take<double>(4);
     t.hist = w.take<long long>(64);
     t.diag = w.take<long long>(2);
@@ -169,7 +178,8 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->use_graph = 1;
     c->jsplit_max_nact = 512;
     c->ipar_small_max_nact = 2048;
-    c->loop_max_nact = 512;
+    c->loop_max_nact = (int64_t)1 << 40;      // every step the scratch allows
+    c->loop_small_nact = 96;
     c->stream = (cudaStream_t)stream;
     gd_carve(&c->d, ws, c->np, c->pcap);
     int dev = 0;
@@ -251,8 +261,9 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
     if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "ipar_small_max_nact")) { c->ipar_small_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "use_graph")) { c->use_graph = value != 0.0; return GD_OK; }
-    if (!strcmp(key, "loop_max_nact")) {
-        c->loop_max_nact = (int64_t)value;
+    if (!strcmp(key, "loop_max_nact") || !strcmp(key, "loop_small_nact")) {
+        if (!strcmp(key, "loop_max_nact")) c->loop_max_nact = (int64_t)value;
+        else c->loop_small_nact = (int64_t)value;
         gd_graph_drop(c);
         return gdk_loop_setup(c);
     }
@@ -548,6 +559,14 @@ extern "C" int gd_get_profile(gd_ctx *c, double *prof_host)
     int rc = gd_prof_drain(c);
     if (rc) return rc;
     memcpy(prof_host, c->prof, sizeof c->prof);
+    return GD_OK;
+}
+
+extern "C" int gd_get_loop_profile(gd_ctx *c, int64_t *out_host)
+{
+    if (!c || !out_host) return GD_EINVAL;
+    GD_CUDA(c, cudaMemcpyAsync(out_host, c->d.lp_ctl + 2, 8 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
     return GD_OK;
 }
 

@@ -50,7 +50,8 @@ struct gd_dev {
     double4 *lp_rec;             // [np + GD_LP_REC_SLACK][2] candidate records, one segment of S rows per CTA
     double *lp_L;                // [256] smallest t_i + dt_i of every CTA's slice
     int *lp_cnt;                 // [256] candidates per CTA
-    unsigned long long *lp_ctl;  // [4] {barrier arrivals, arrivals at the start of the current launch, particle steps in the loop, -}
+    unsigned long long *lp_ctl;  // [16] {barrier arrivals, arrivals at the start of the current launch, then profiling counters:
+                                 //  particle steps, block steps, ns in the loop, ns per phase x 4, launches that ran}
 };
 
 #define GD_SCAN_MAX_BLOCKS 1024
@@ -82,7 +83,8 @@ struct gd_ctx {
     gd_ctrl *h_ctrl;                     // pinned host mirror of d.ctrl
     int use_graph;
     int64_t loop_max_nact;               // option: largest active set the persistent loop takes (0 = loop off)
-    int loop_grid, loop_S, loop_hi;      // geometry of k_block_loop (loop_grid = 0: not usable)
+    int64_t loop_small_nact;             // option: active sets up to this size use the lanes-over-sources mapping
+    int loop_grid, loop_S, loop_hi, loop_cap;   // geometry of k_block_loop (loop_grid = 0: not usable)
     size_t loop_smem;
     int64_t graph_nodes;                 // kernel nodes in step_graph
     int sm_count;

@@ -36,25 +36,19 @@ k_correct_timestep(gd_dev d, int n_act, double t_next, double eta, double dt_min
         const double *a1 = d.a1 + 3 * (int64_t)k, *j1 = d.j1 + 3 * (int64_t)k;
         double a1x = a1[0], a1y = a1[1], a1z = a1[2], j1x = j1[0], j1y = j1[1], j1z = j1[2];
 
-        const double h = ad.w;
-        const gd_hpow hp = gd_step_powers(h);
-        gd_corr1 cx = gd_correct_component(pxy.x, pvxy.x, ad.x, jk.x, a1x, j1x, hp);
-        gd_corr1 cy = gd_correct_component(pxy.y, pvxy.y, ad.y, jk.y, a1y, j1y, hp);
-        gd_corr1 cz = gd_correct_component(pzm.x, pvz, ad.z, jk.z, a1z, j1z, hp);
-
-        double na1 = gd_norm3(a1x, a1y, a1z), nj1 = gd_norm3(j1x, j1y, j1z);
-        double na2 = gd_norm3(cx.a2e, cy.a2e, cz.a2e), na3 = gd_norm3(cx.a3, cy.a3, cz.a3);
-        int flags;
-        const double dnew = gd_new_step(na1, nj1, na2, na3, h, t_next, eta, dt_min, dt_max, halving_mode, flags);
-        if (flags & 1) atomicAdd(&s_diag[0], 1u);
-        if (flags & 2) atomicAdd(&s_diag[1], 1u);
+        const double a1v[3] = {a1x, a1y, a1z}, j1v[3] = {j1x, j1y, j1z};
+        const gd_corrected r = gd_correct_particle(pxy.x, pxy.y, pzm.x, pvxy.x, pvxy.y, pvz, ad, jk, a1v, j1v, t_next, eta, dt_min,
+                                                   dt_max, halving_mode);
+        const double dnew = r.dt;
+        if (r.flags & 1) atomicAdd(&s_diag[0], 1u);
+        if (r.flags & 2) atomicAdd(&s_diag[1], 1u);
 
         // level of the step just taken: h = 2^-lvl
-        int lvl = gd_step_level(h);
+        int lvl = gd_step_level(ad.w);
         if (lvl >= 0 && lvl < 64) atomicAdd(&s_hist[lvl], 1u);
 
-        d.xm[i] = make_double4(cx.xnew, cy.xnew, cz.xnew, pzm.y);
-        d.vt[i] = make_double4(cx.vnew, cy.vnew, cz.vnew, t_next);
+        d.xm[i] = make_double4(r.x, r.y, r.z, pzm.y);
+        d.vt[i] = make_double4(r.vx, r.vy, r.vz, t_next);
         d.ad[i] = make_double4(a1x, a1y, a1z, dnew);
         d.jk[i] = make_double4(j1x, j1y, j1z, 0.0);
         d.tnext[i] = t_next + dnew;                           // exact (dyadic)

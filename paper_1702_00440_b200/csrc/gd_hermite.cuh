@@ -96,3 +96,25 @@ __device__ __forceinline__ double gd_new_step(double na1, double nj1, double na2
 
 // level of a step h = 2^-lvl
 __device__ __forceinline__ int gd_step_level(double h) { return 1023 - (int)((__double_as_longlong(h) >> 52) & 0x7ff); }
+
+// ---- the whole per-particle update: corrector (3 components) + criterion + block rule ---------------------------
+struct gd_corrected { double x, y, z, vx, vy, vz, dt; int flags; };
+
+__device__ __forceinline__ gd_corrected gd_correct_particle(double xp, double yp, double zp, double vxp, double vyp, double vzp,
+                                                            const double4 &ad, const double4 &jk, const double (&a1)[3],
+                                                            const double (&j1)[3], double t_next, double eta, double dt_min,
+                                                            double dt_max, int halving_mode)
+{
+    const double h = ad.w;
+    const gd_hpow hp = gd_step_powers(h);
+    const gd_corr1 cx = gd_correct_component(xp, vxp, ad.x, jk.x, a1[0], j1[0], hp);
+    const gd_corr1 cy = gd_correct_component(yp, vyp, ad.y, jk.y, a1[1], j1[1], hp);
+    const gd_corr1 cz = gd_correct_component(zp, vzp, ad.z, jk.z, a1[2], j1[2], hp);
+    const double na1 = gd_norm3(a1[0], a1[1], a1[2]), nj1 = gd_norm3(j1[0], j1[1], j1[2]);
+    const double na2 = gd_norm3(cx.a2e, cy.a2e, cz.a2e), na3 = gd_norm3(cx.a3, cy.a3, cz.a3);
+    gd_corrected r;
+    r.dt = gd_new_step(na1, nj1, na2, na3, h, t_next, eta, dt_min, dt_max, halving_mode, r.flags);
+    r.x = cx.xnew; r.y = cy.xnew; r.z = cz.xnew;
+    r.vx = cx.vnew; r.vy = cy.vnew; r.vz = cz.vnew;
+    return r;
+}

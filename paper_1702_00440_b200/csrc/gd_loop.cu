@@ -27,17 +27,24 @@
 #include "gd_common.cuh"
 #include "gd_hermite.cuh"
 #include "gd_pair.cuh"
+#include <limits.h>
 
 #define GD_LP_THREADS 256
 #define GD_LP_WARPS (GD_LP_THREADS / 32)
 #define GD_LP_MAX_GRID 256          // CTAs (one per SM); bounds the shared tables
-#define GD_LP_MAX_HI 1024           // largest active set the loop takes
+#define GD_LP_MAX_SMALL 256         // largest active set of the lanes-over-sources mapping (bounds the position map)
 
 struct gd_largs {
-    int np, S, hi;
+    int n;                           // particles; CTA c owns [c n / G, (c + 1) n / G)
+    int S;                           // slice capacity in shared memory (multiple of 32)
+    int hi;                          // largest active set the loop takes
+    int cap;                         // row length of the partial sums: partial[c][comp][cap]
+    int small_hi;                    // n_act <= small_hi: lanes over sources; above: lanes over sinks
     double eps2, eta, dt_min, dt_max;
     int halving_mode;
 };
+
+__device__ __forceinline__ int gd_slice_begin(int c, int n, int G) { return (int)((long long)c * n / G); }
 
 #define GD_INF __longlong_as_double(0x7ff0000000000000LL)
 #define GD_FULL 0xffffffffu
@@ -60,6 +67,13 @@ __device__ __forceinline__ void gd_bar_wait(unsigned long long *bar, unsigned lo
         } while (v < target);
     }
     __syncthreads();
+}
+
+__device__ __forceinline__ unsigned long long gd_gtime()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
 }
 
 __device__ __forceinline__ double gd_warp_min_d(double v)
@@ -117,26 +131,25 @@ __device__ __forceinline__ int gd_rs6_elem(int lane)
 
 // ---- shared memory of one CTA ----------------------------------------------------------------------------------------
 struct gd_lsm {
-    double2 *pxy, *pzm, *vxy;        // [S] predicted records of the own slice (at t+ during [force] / [correct])
-    double *vz;                      // [S]
-    double *ts;                      // [S] t_i + dt_i of the own slice (+inf beyond np and in the padding)
+    double2 *pxy, *pzm, *vxy;        // [S] predicted records of the own slice (at t+ during [force] / [correct]);
+    double *vz;                      // [S]   entries beyond the slice are zero-mass padding up to a multiple of 32
+    double *ts;                      // [S] t_i + dt_i of the own slice
     int *lact;                       // [S] local indices of the own candidates, ascending
-    int *smap;                       // [hi] active list position -> row of `rec`
-    double *sL;                      // [GD_LP_MAX_GRID] L_c of every CTA
+    int *smap;                       // [GD_LP_MAX_SMALL] active list position -> row of `rec` (small mode)
     int *spre;                       // [GD_LP_MAX_GRID + 1] exclusive prefix of the contributing candidate counts
-    double *red;                     // [GD_LP_WARPS][32] warp partial sums of a split evaluation
+    double *red;                     // [GD_LP_WARPS][6][32] warp partial sums of a split evaluation
     double *wmin;                    // [GD_LP_WARPS]
     int *wcnt;                       // [GD_LP_WARPS + 1]
     unsigned int *hist;              // [64] particle steps per level, [64..65] diagnostics
 };
 
-__host__ __device__ inline size_t gd_lsm_bytes(int S, int hi)
+__host__ __device__ inline size_t gd_lsm_bytes(int S)
 {
-    return (size_t)S * (16 * 3 + 8 + 8 + 4) + (size_t)hi * 4 + GD_LP_MAX_GRID * 8 + (GD_LP_MAX_GRID + 1) * 4 + 4 +
-           GD_LP_WARPS * 32 * 8 + GD_LP_WARPS * 8 + (GD_LP_WARPS + 1) * 4 + 4 + 66 * 4 + 64;
+    return (size_t)S * (16 * 3 + 8 + 8 + 4) + GD_LP_WARPS * 6 * 32 * 8 + GD_LP_WARPS * 8 + GD_LP_MAX_SMALL * 4 +
+           (GD_LP_MAX_GRID + 1) * 4 + (GD_LP_WARPS + 1) * 4 + 66 * 4 + 64;
 }
 
-__device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S, int hi)
+__device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S)
 {
     gd_lsm s;
     unsigned char *p = base;
@@ -145,11 +158,10 @@ __device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S, int h
     s.vxy = (double2 *)p; p += (size_t)S * 16;
     s.vz = (double *)p; p += (size_t)S * 8;
     s.ts = (double *)p; p += (size_t)S * 8;
-    s.sL = (double *)p; p += GD_LP_MAX_GRID * 8;
-    s.red = (double *)p; p += GD_LP_WARPS * 32 * 8;
+    s.red = (double *)p; p += GD_LP_WARPS * 6 * 32 * 8;
     s.wmin = (double *)p; p += GD_LP_WARPS * 8;
     s.lact = (int *)p; p += (size_t)S * 4;
-    s.smap = (int *)p; p += (size_t)hi * 4;
+    s.smap = (int *)p; p += GD_LP_MAX_SMALL * 4;
     s.spre = (int *)p; p += (GD_LP_MAX_GRID + 1) * 4;
     s.wcnt = (int *)p; p += (GD_LP_WARPS + 1) * 4;
     s.hist = (unsigned int *)p;
@@ -207,8 +219,16 @@ __device__ __forceinline__ int gd_publish(const gd_dev &d, const gd_lsm &sm, int
     return cnt;
 }
 
-// ---- [force]: BI sinks (active-list positions pos0 .. pos0 + BI - 1) against the source rounds [r_begin, r_end) -------
-// of the own slice; lane l takes source 32 r + l.  Returns the 6 BI per-lane sums in v[b * 6 + {ax, ay, az, jx, jy, jz}].
+__device__ __forceinline__ gd_src gd_lp_load_sink(const gd_dev &d, int row_index)
+{
+    const double2 *row = reinterpret_cast<const double2 *>(d.lp_rec + 2 * (size_t)row_index);
+    const double2 xy = __ldcg(row), zi = __ldcg(row + 1), wxy = __ldcg(row + 2), wz = __ldcg(row + 3);
+    return gd_src{xy.x, xy.y, zi.x, 0.0, wxy.x, wxy.y, wz.x};
+}
+
+// ---- [force], small mode: lanes stride over the own sources ------------------------------------------------------------
+// BI sinks (active-list positions pos0 .. pos0 + BI - 1) against the source rounds [r_begin, r_end) of the own
+// slice; lane l takes source 32 r + l.  Returns the 6 BI per-lane sums in v[b * 6 + {ax, ay, az, jx, jy, jz}].
 template <int BI, bool EPS0>
 __device__ __forceinline__ void gd_lp_item(const gd_dev &d, const gd_lsm &sm, int pos0, int r_begin, int r_end, int lane,
                                            double eps2, double *v)
@@ -217,9 +237,7 @@ __device__ __forceinline__ void gd_lp_item(const gd_dev &d, const gd_lsm &sm, in
     gd_acc acc[BI];
 #pragma unroll
     for (int b = 0; b < BI; ++b) {
-        const double2 *row = reinterpret_cast<const double2 *>(d.lp_rec + 2 * (size_t)sm.smap[pos0 + b]);
-        const double2 xy = __ldcg(row), zi = __ldcg(row + 1), wxy = __ldcg(row + 2), wz = __ldcg(row + 3);
-        si[b] = gd_src{xy.x, xy.y, zi.x, 0.0, wxy.x, wxy.y, wz.x};
+        si[b] = gd_lp_load_sink(d, sm.smap[pos0 + b]);
         acc[b] = gd_acc{0, 0, 0, 0, 0, 0};
     }
 #pragma unroll 2
@@ -237,16 +255,22 @@ __device__ __forceinline__ void gd_lp_item(const gd_dev &d, const gd_lsm &sm, in
     }
 }
 
+// element e = b * 6 + comp of the block starting at position pos -> partial[me][comp][pos + b]
+__device__ __forceinline__ void gd_lp_put(double *out, int cap, int pos, int e, double val)
+{
+    const int b = e / 6, comp = e - 6 * b;
+    out[(size_t)comp * cap + pos + b] = val;
+}
+
 // One work item = a register block of sinks: items 0 .. n4 - 1 hold 4 sinks, the n_act % 4 last ones hold 1.
-// items >= warps: warp w takes items w, w + 8, ... over all source rounds and writes partial[me][pos][6] itself.
+// items >= warps: warp w takes items w, w + 8, ... over all source rounds and writes its sums itself.
 // items <  warps: the rounds of every item are split over nsplit = 8 / items warps; the warp sums meet in shared
 //                 memory and are added in chunk order.
 template <bool EPS0>
-__device__ __forceinline__ void gd_lp_force(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, int me, int n_act, int rounds)
+__device__ __forceinline__ void gd_lp_force_small(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int n_act, int rounds)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n4 = n_act >> 2, items = n4 + (n_act & 3);
-    double *out = d.partial + (size_t)me * la.hi * 6;
     if (items >= GD_LP_WARPS) {
         for (int it = warp; it < items; it += GD_LP_WARPS) {
             if (it < n4) {
@@ -254,14 +278,14 @@ __device__ __forceinline__ void gd_lp_force(const gd_dev &d, const gd_lsm &sm, c
                 gd_lp_item<4, EPS0>(d, sm, 4 * it, 0, rounds, lane, la.eps2, v);
                 gd_rs24(v, lane);
                 const int e = gd_rs24_elem(lane);
-                if (e >= 0) out[(size_t)(4 * it) * 6 + e] = v[0];
+                if (e >= 0) gd_lp_put(out, la.cap, 4 * it, e, v[0]);
             } else {
                 double v[6];
                 const int pos = 4 * n4 + (it - n4);
                 gd_lp_item<1, EPS0>(d, sm, pos, 0, rounds, lane, la.eps2, v);
                 gd_rs6(v, lane);
                 const int e = gd_rs6_elem(lane);
-                if (e >= 0) out[(size_t)pos * 6 + e] = v[0];
+                if (e >= 0) gd_lp_put(out, la.cap, pos, e, v[0]);
             }
         }
         return;
@@ -291,30 +315,125 @@ __device__ __forceinline__ void gd_lp_force(const gd_dev &d, const gd_lsm &sm, c
     if (work && chunk == 0 && lane < (four ? 24 : 6)) {
         double s = sm.red[warp * 32 + lane];
         for (int c = 1; c < nsplit; ++c) s += sm.red[(warp + c) * 32 + lane];
-        out[(size_t)pos * 6 + lane] = s;
+        gd_lp_put(out, la.cap, pos, lane, s);
     }
 }
 
-// ---- [correct]: one warp per own active particle -------------------------------------------------------------------------
-// Lanes stride over the CTAs' partial rows (ascending c within a lane, fixed butterfly across lanes); lanes 0..2
-// then run one Cartesian component of the corrector each; the criterion and the block rule are evaluated by every
-// lane on the same values; lane 0 commits.
-__device__ __forceinline__ void gd_lp_correct(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, int G, int p0, int pos, int p,
-                                              double t_next, int lane)
+// ---- [force], big mode: lanes hold sinks, the own sources are read by broadcast --------------------------------------
+// Tile = 32 consecutive active-list positions.  tiles >= warps: warp w takes tiles w, w + 8, ... against the whole
+// slice; fewer tiles: the slice is split over nsplit = 8 / tiles warps per tile and the warp sums are added in chunk
+// order in shared memory.  Two independent accumulator sets (even / odd sources) keep the FP64 pipe fed.
+template <bool EPS0>
+__device__ __forceinline__ gd_acc gd_lp_tile(const gd_lsm &sm, const gd_src &si, int jb, int je, double eps2)
 {
+    gd_acc a0 = gd_acc{0, 0, 0, 0, 0, 0}, a1 = gd_acc{0, 0, 0, 0, 0, 0};
+    int j = jb;
+#pragma unroll 2
+    for (; j + 1 < je; j += 2) {
+        const double2 xy0 = sm.pxy[j], zm0 = sm.pzm[j], vxy0 = sm.vxy[j];
+        const double2 xy1 = sm.pxy[j + 1], zm1 = sm.pzm[j + 1], vxy1 = sm.vxy[j + 1];
+        const gd_src s0{xy0.x, xy0.y, zm0.x, zm0.y, vxy0.x, vxy0.y, sm.vz[j]};
+        const gd_src s1{xy1.x, xy1.y, zm1.x, zm1.y, vxy1.x, vxy1.y, sm.vz[j + 1]};
+        gd_pair<EPS0>(si, s0, eps2, a0);
+        gd_pair<EPS0>(si, s1, eps2, a1);
+    }
+    if (j < je) {
+        const double2 xy0 = sm.pxy[j], zm0 = sm.pzm[j], vxy0 = sm.vxy[j];
+        const gd_src s0{xy0.x, xy0.y, zm0.x, zm0.y, vxy0.x, vxy0.y, sm.vz[j]};
+        gd_pair<EPS0>(si, s0, eps2, a0);
+    }
+    a0.ax += a1.ax; a0.ay += a1.ay; a0.az += a1.az;
+    a0.jx += a1.jx; a0.jy += a1.jy; a0.jz += a1.jz;
+    return a0;
+}
+
+// position in the active list -> row of rec: CTA c with spre[c] <= pos < spre[c + 1] (segments of empty CTAs have
+// zero width), row = first row of c's segment + offset
+__device__ __forceinline__ int gd_lp_row_of(const gd_lsm &sm, int pos, int n, int G)
+{
+    int lo = 0, hi = G;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (sm.spre[mid] <= pos) lo = mid; else hi = mid;
+    }
+    return gd_slice_begin(lo, n, G) + (pos - sm.spre[lo]);
+}
+
+template <bool EPS0>
+__device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int G, int n_act, int cnt_own)
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tiles = (n_act + 31) >> 5;
+    if (tiles >= GD_LP_WARPS) {
+        for (int tile = warp; tile < tiles; tile += GD_LP_WARPS) {
+            const int pos = tile * 32 + lane;
+            const gd_src si = gd_lp_load_sink(d, gd_lp_row_of(sm, min(pos, n_act - 1), la.n, G));
+            const gd_acc a = gd_lp_tile<EPS0>(sm, si, 0, cnt_own, la.eps2);
+            if (pos < n_act) {
+                out[pos] = a.ax; out[(size_t)la.cap + pos] = a.ay; out[(size_t)2 * la.cap + pos] = a.az;
+                out[(size_t)3 * la.cap + pos] = a.jx; out[(size_t)4 * la.cap + pos] = a.jy; out[(size_t)5 * la.cap + pos] = a.jz;
+            }
+        }
+        return;
+    }
+    const int nsplit = GD_LP_WARPS / tiles;
+    const int tile = warp / nsplit, chunk = warp - tile * nsplit;
+    const bool work = tile < tiles;
+    const int pos = tile * 32 + lane;
+    if (work) {
+        const gd_src si = gd_lp_load_sink(d, gd_lp_row_of(sm, min(pos, n_act - 1), la.n, G));
+        const int jb = (int)((long long)cnt_own * chunk / nsplit), je = (int)((long long)cnt_own * (chunk + 1) / nsplit);
+        const gd_acc a = gd_lp_tile<EPS0>(sm, si, jb, je, la.eps2);
+        double *r = sm.red + warp * 192 + lane;
+        r[0] = a.ax; r[32] = a.ay; r[64] = a.az; r[96] = a.jx; r[128] = a.jy; r[160] = a.jz;
+    }
+    __syncthreads();
+    if (work && chunk == 0 && pos < n_act) {
+#pragma unroll
+        for (int comp = 0; comp < 6; ++comp) {
+            double s = sm.red[warp * 192 + comp * 32 + lane];
+            for (int c = 1; c < nsplit; ++c) s += sm.red[(warp + c) * 192 + comp * 32 + lane];
+            out[(size_t)comp * la.cap + pos] = s;
+        }
+    }
+}
+
+// ---- [correct] -----------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void gd_lp_commit(const gd_dev &d, const gd_lsm &sm, int i, int p, double m, const gd_corrected &r,
+                                             const double (&a1)[3], const double (&j1)[3], double h, double t_next)
+{
+    if (r.flags & 1) atomicAdd(&sm.hist[64], 1u);
+    if (r.flags & 2) atomicAdd(&sm.hist[65], 1u);
+    const int lvl = gd_step_level(h);
+    if (lvl >= 0 && lvl < 64) atomicAdd(&sm.hist[lvl], 1u);
+    d.xm[i] = make_double4(r.x, r.y, r.z, m);
+    d.vt[i] = make_double4(r.vx, r.vy, r.vz, t_next);
+    d.ad[i] = make_double4(a1[0], a1[1], a1[2], r.dt);
+    d.jk[i] = make_double4(j1[0], j1[1], j1[2], 0.0);
+    const double tn = t_next + r.dt;                         // exact (dyadic)
+    d.tnext[i] = tn;
+    sm.ts[p] = tn;
+}
+
+// small mode: one warp per own active particle.  Lanes stride over the CTAs' partial sums (ascending c within a lane,
+// fixed butterfly across lanes); lanes 0..2 then run one Cartesian component of the corrector each; the criterion and
+// the block rule are evaluated by every lane on the same values; lane 0 commits.
+__device__ __forceinline__ void gd_lp_correct_warp(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, int G, int p0, int pos, int p,
+                                                   double t_next, int lane)
+{
+    const int i = p0 + p;
+    const double4 ad = d.ad[i], jk = d.jk[i];
     double s[6] = {0, 0, 0, 0, 0, 0};
     for (int c = lane; c < G; c += 32) {
-        const double2 *row = reinterpret_cast<const double2 *>(d.partial + ((size_t)c * la.hi + pos) * 6);
-        const double2 u0 = __ldcg(row), u1 = __ldcg(row + 1), u2 = __ldcg(row + 2);
-        s[0] += u0.x; s[1] += u0.y; s[2] += u1.x; s[3] += u1.y; s[4] += u2.x; s[5] += u2.y;
+        const double *row = d.partial + (size_t)c * 6 * la.cap + pos;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) s[k] += __ldcg(row + (size_t)k * la.cap);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
         for (int k = 0; k < 6; ++k) s[k] += __shfl_xor_sync(GD_FULL, s[k], o);
     }
-    const int i = p0 + p;
-    const double4 ad = d.ad[i], jk = d.jk[i];
     const double2 pxy = sm.pxy[p], pzm = sm.pzm[p], pvxy = sm.vxy[p];
     const double pvz = sm.vz[p];
     const int comp = lane < 2 ? lane : 2;
@@ -329,29 +448,43 @@ __device__ __forceinline__ void gd_lp_correct(const gd_dev &d, const gd_lsm &sm,
     const gd_corr1 cr = gd_correct_component(xp, vp, a0, j0, a1, j1, hp);
     const double a2x = __shfl_sync(GD_FULL, cr.a2e, 0), a2y = __shfl_sync(GD_FULL, cr.a2e, 1), a2z = __shfl_sync(GD_FULL, cr.a2e, 2);
     const double a3x = __shfl_sync(GD_FULL, cr.a3, 0), a3y = __shfl_sync(GD_FULL, cr.a3, 1), a3z = __shfl_sync(GD_FULL, cr.a3, 2);
-    const double xn = __shfl_sync(GD_FULL, cr.xnew, 0), yn = __shfl_sync(GD_FULL, cr.xnew, 1), zn = __shfl_sync(GD_FULL, cr.xnew, 2);
-    const double vxn = __shfl_sync(GD_FULL, cr.vnew, 0), vyn = __shfl_sync(GD_FULL, cr.vnew, 1), vzn = __shfl_sync(GD_FULL, cr.vnew, 2);
+    gd_corrected r;
+    r.x = __shfl_sync(GD_FULL, cr.xnew, 0); r.y = __shfl_sync(GD_FULL, cr.xnew, 1); r.z = __shfl_sync(GD_FULL, cr.xnew, 2);
+    r.vx = __shfl_sync(GD_FULL, cr.vnew, 0); r.vy = __shfl_sync(GD_FULL, cr.vnew, 1); r.vz = __shfl_sync(GD_FULL, cr.vnew, 2);
     const double na1 = gd_norm3(s[0], s[1], s[2]), nj1 = gd_norm3(s[3], s[4], s[5]);
     const double na2 = gd_norm3(a2x, a2y, a2z), na3 = gd_norm3(a3x, a3y, a3z);
-    int flags;
-    const double dnew = gd_new_step(na1, nj1, na2, na3, h, t_next, la.eta, la.dt_min, la.dt_max, la.halving_mode, flags);
+    r.dt = gd_new_step(na1, nj1, na2, na3, h, t_next, la.eta, la.dt_min, la.dt_max, la.halving_mode, r.flags);
     if (lane == 0) {
-        if (flags & 1) atomicAdd(&sm.hist[64], 1u);
-        if (flags & 2) atomicAdd(&sm.hist[65], 1u);
-        const int lvl = gd_step_level(h);
-        if (lvl >= 0 && lvl < 64) atomicAdd(&sm.hist[lvl], 1u);
-        d.xm[i] = make_double4(xn, yn, zn, pzm.y);
-        d.vt[i] = make_double4(vxn, vyn, vzn, t_next);
-        d.ad[i] = make_double4(s[0], s[1], s[2], dnew);
-        d.jk[i] = make_double4(s[3], s[4], s[5], 0.0);
-        const double tn = t_next + dnew;                     // exact (dyadic)
-        d.tnext[i] = tn;
-        sm.ts[p] = tn;
+        const double a1v[3] = {s[0], s[1], s[2]}, j1v[3] = {s[3], s[4], s[5]};
+        gd_lp_commit(d, sm, i, p, pzm.y, r, a1v, j1v, h, t_next);
     }
 }
 
+// big mode: one thread per own active particle; the CTAs' partial sums are added in ascending c
+__device__ __forceinline__ void gd_lp_correct_thread(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, int G, int p0, int pos, int p,
+                                                     double t_next)
+{
+    const int i = p0 + p;
+    const double4 ad = d.ad[i], jk = d.jk[i];
+    double s[6] = {0, 0, 0, 0, 0, 0};
+    const double *row = d.partial + pos;
+    const size_t cs = (size_t)6 * la.cap;
+#pragma unroll 4
+    for (int c = 0; c < G; ++c) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) s[k] += __ldcg(row + (size_t)c * cs + (size_t)k * la.cap);
+    }
+    const double2 pxy = sm.pxy[p], pzm = sm.pzm[p], pvxy = sm.vxy[p];
+    const double pvz = sm.vz[p];
+    const double a1v[3] = {s[0], s[1], s[2]}, j1v[3] = {s[3], s[4], s[5]};
+    const gd_corrected r = gd_correct_particle(pxy.x, pxy.y, pzm.x, pvxy.x, pvxy.y, pvz, ad, jk, a1v, j1v, t_next, la.eta, la.dt_min,
+                                               la.dt_max, la.halving_mode);
+    gd_lp_commit(d, sm, i, p, pzm.y, r, a1v, j1v, ad.w, t_next);
+}
+
 // ---------------------------------------------------------------------------------------------------------------------------
-// lp_ctl[0] = barrier arrivals (monotonic over the life of the context), lp_ctl[1] = arrivals when this launch began.
+// lp_ctl[0] = barrier arrivals (monotonic over the life of the context), lp_ctl[1] = arrivals when this launch began,
+// lp_ctl[2..9] = profiling counters (gd_get_loop_profile).
 template <bool EPS0>
 __global__ void __launch_bounds__(GD_LP_THREADS, 1)
 k_block_loop(gd_dev d, gd_largs la)
@@ -359,20 +492,31 @@ k_block_loop(gd_dev d, gd_largs la)
     extern __shared__ __align__(16) unsigned char gd_lp_smem[];
     gd_ctrl *ct = d.ctrl;
     if (ct->finished) return;                                // nobody writes ct before the first barrier
-    const gd_lsm sm = gd_lsm_carve(gd_lp_smem, la.S, la.hi);
+    const gd_lsm sm = gd_lsm_carve(gd_lp_smem, la.S);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = gridDim.x, me = blockIdx.x;
-    const int p0 = me * la.S;
-    const int cnt_own = max(0, min(la.S, la.np - p0));       // multiple of 32
-    const int rounds = cnt_own / 32;
+    const int p0 = gd_slice_begin(me, la.n, G);
+    const int cnt_own = gd_slice_begin(me + 1, la.n, G) - p0;
+    const int rounds = (cnt_own + 31) / 32;
     const double t_end = ct->t_end;
     const long long max_steps = ct->max_steps;
     double t_cur = ct->t;
     long long steps = ct->steps, psteps = 0;
+    const long long ct_steps0 = steps;
     unsigned long long *bar = d.lp_ctl;
     unsigned long long target = d.lp_ctl[1];
+    double *out = d.partial + (size_t)me * 6 * la.cap;
 
-    for (int p = tid; p < cnt_own; p += GD_LP_THREADS) sm.ts[p] = d.tnext[p0 + p];
+    for (int p = tid; p < rounds * 32; p += GD_LP_THREADS) {
+        if (p < cnt_own) {
+            sm.ts[p] = d.tnext[p0 + p];
+        } else {                                             // zero-mass padding of the last source round
+            sm.pxy[p] = make_double2(0.0, 0.0);
+            sm.pzm[p] = make_double2(0.0, 0.0);
+            sm.vxy[p] = make_double2(0.0, 0.0);
+            sm.vz[p] = 0.0;
+        }
+    }
     if (tid < 66) sm.hist[tid] = 0u;
     __syncthreads();
     double L_me;
@@ -382,6 +526,8 @@ k_block_loop(gd_dev d, gd_largs la)
     gd_bar_wait(bar, target);
 
     bool fin = false;
+    unsigned long long tr[4] = {0, 0, 0, 0}, g0 = gd_gtime(), g1;   // CTA 0's view: ns in [force], barrier, [correct], barrier
+    const unsigned long long g_begin = g0;
     for (;;) {
         if (t_cur >= t_end || (max_steps >= 0 && steps >= max_steps)) { fin = true; break; }
         // ---- [force] ----
@@ -403,9 +549,14 @@ k_block_loop(gd_dev d, gd_largs la)
 #pragma unroll
         for (int w = 0; w < GD_LP_WARPS; ++w) { int c = sm.wcnt[w]; wbase += (w < warp) ? c : 0; n_act += c; }
         if (n_act > la.hi) break;                            // uniform: the stage kernels take this step
+        const bool small = n_act <= la.small_hi;
         const int excl = wbase + incl - mine;
         if (tid < G) sm.spre[tid] = excl;
-        for (int k = 0; k < mine; ++k) sm.smap[excl + k] = tid * la.S + k;
+        if (tid == 0) sm.spre[G] = n_act;
+        if (small && mine > 0) {
+            const int r0 = gd_slice_begin(tid, la.n, G);
+            for (int k = 0; k < mine; ++k) sm.smap[excl + k] = r0 + k;
+        }
         // own slice predicted to t+
         for (int p = tid; p < cnt_own; p += GD_LP_THREADS) {
             const int i = p0 + p;
@@ -417,24 +568,33 @@ k_block_loop(gd_dev d, gd_largs la)
             sm.vz[p] = q.vz;
         }
         __syncthreads();
-        gd_lp_force<EPS0>(d, sm, la, me, n_act, rounds);
+        if (small) gd_lp_force_small<EPS0>(d, sm, la, out, n_act, rounds);
+        else gd_lp_force_big<EPS0>(d, sm, la, out, G, n_act, cnt_own);
+        g1 = gd_gtime(); tr[0] += g1 - g0; g0 = g1;
         gd_bar_arrive(bar);
         target += G;
         gd_bar_wait(bar, target);
+        g1 = gd_gtime(); tr[1] += g1 - g0; g0 = g1;
         // ---- [correct] + [publish] ----
         const bool contributing = (L_me == t_next) && cnt_me > 0;
         if (contributing) {
             const int pre = sm.spre[me];
-            for (int k = warp; k < cnt_me; k += GD_LP_WARPS) gd_lp_correct(d, sm, la, G, p0, pre + k, sm.lact[k], t_next, lane);
+            if (small) {
+                for (int k = warp; k < cnt_me; k += GD_LP_WARPS) gd_lp_correct_warp(d, sm, la, G, p0, pre + k, sm.lact[k], t_next, lane);
+            } else {
+                for (int k = tid; k < cnt_me; k += GD_LP_THREADS) gd_lp_correct_thread(d, sm, la, G, p0, pre + k, sm.lact[k], t_next);
+            }
             __syncthreads();
             cnt_me = gd_publish(d, sm, me, p0, cnt_own, &L_me);
         }
         t_cur = t_next;
         steps += 1;
         psteps += n_act;
+        g1 = gd_gtime(); tr[2] += g1 - g0; g0 = g1;
         gd_bar_arrive(bar);
         target += G;
         gd_bar_wait(bar, target);
+        g1 = gd_gtime(); tr[3] += g1 - g0; g0 = g1;
     }
 
     // ---- leave: flush the counters; CTA 0 hands the run state back ----
@@ -446,31 +606,35 @@ k_block_loop(gd_dev d, gd_largs la)
         ct->psteps += psteps;
         if (fin) ct->finished = 1;
         d.lp_ctl[1] = target;
-        d.lp_ctl[2] += (unsigned long long)psteps;           // particle steps taken inside the loop (profiling)
+        // profiling counters: particle steps and block steps taken inside the loop, ns inside it, ns per phase
+        d.lp_ctl[2] += (unsigned long long)psteps;
+        d.lp_ctl[3] += (unsigned long long)(steps - ct_steps0);
+        d.lp_ctl[4] += gd_gtime() - g_begin;
+        for (int k = 0; k < 4; ++k) d.lp_ctl[5 + k] += tr[k];
+        d.lp_ctl[9] += 1ull;
     }
 }
 
 // ---- host side ------------------------------------------------------------------------------------------------------------
-// Geometry: one CTA per SM; S = slice length (multiple of 32); hi = largest active set taken, bounded by the option
-// `loop_max_nact`, the partial-sum scratch (grid x hi rows) and GD_LP_MAX_HI.  loop_grid = 0: the loop is not usable
+// Geometry: one CTA per SM; S = slice capacity (multiple of 32); hi = largest active set taken, bounded by the option
+// `loop_max_nact` and by the partial-sum scratch (grid x 6 x cap doubles).  loop_grid = 0: the loop is not usable
 // (slice does not fit in shared memory, or the device cannot co-schedule the grid) and the stage kernels run alone.
 int gdk_loop_setup(gd_ctx *c)
 {
     c->loop_grid = 0;
     int grid = c->sm_count < GD_LP_MAX_GRID ? c->sm_count : GD_LP_MAX_GRID;
-    if (grid < 1 || c->loop_max_nact < 1) return 0;
-    int64_t S = (c->np + grid - 1) / grid;
+    if (grid < 1 || c->loop_max_nact < 1 || c->n > INT_MAX / 2) return 0;
+    int64_t S = (c->n + grid - 1) / grid;
     S = (S + 31) / 32 * 32;
-    if (S * grid > c->np + GD_LP_REC_SLACK) return 0;
-    int64_t hi = c->loop_max_nact;
-    if (hi > GD_LP_MAX_HI) hi = GD_LP_MAX_HI;
-    if (hi > c->pcap / grid) hi = c->pcap / grid;
+    int64_t hi = c->loop_max_nact < c->n ? c->loop_max_nact : c->n;
+    int64_t cap = (hi + 31) / 32 * 32;
+    if (cap > c->pcap / grid) { cap = c->pcap / grid / 32 * 32; hi = cap; }
     if (hi < 1) return 0;
     int dev = 0, max_smem = 0, coop = 0;
     GD_CUDA(c, cudaGetDevice(&dev));
     GD_CUDA(c, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     GD_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
-    const size_t bytes = gd_lsm_bytes((int)S, (int)hi);
+    const size_t bytes = gd_lsm_bytes((int)S);
     if (!coop || bytes > (size_t)max_smem) return 0;
     GD_CUDA(c, cudaFuncSetAttribute(k_block_loop<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     GD_CUDA(c, cudaFuncSetAttribute(k_block_loop<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
@@ -480,6 +644,7 @@ int gdk_loop_setup(gd_ctx *c)
     c->loop_grid = grid;
     c->loop_S = (int)S;
     c->loop_hi = (int)hi;
+    c->loop_cap = (int)cap;
     c->loop_smem = bytes;
     return 0;
 }
@@ -489,9 +654,12 @@ int gdk_loop(gd_ctx *c)
 {
     if (c->loop_grid < 1) return 0;
     gd_largs la;
-    la.np = (int)c->np;
+    la.n = (int)c->n;
     la.S = c->loop_S;
     la.hi = c->loop_hi;
+    la.cap = c->loop_cap;
+    int64_t sh = c->loop_small_nact < GD_LP_MAX_SMALL ? c->loop_small_nact : GD_LP_MAX_SMALL;
+    la.small_hi = (int)(sh < 0 ? 0 : sh);
     la.eps2 = c->eps2;
     la.eta = c->eta;
     la.dt_min = c->dt_min;

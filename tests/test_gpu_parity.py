@@ -357,8 +357,8 @@ def test_loop_first_100_block_steps_bit_exact_schedule(gd, cfg, n):
     h.close()
 
 
-@pytest.mark.parametrize("hi", [1, 3, 8, 64, 1024])
-def test_loop_threshold_sweep_same_schedule(gd, hi):
+@pytest.mark.parametrize("hi,small", [(1, 96), (3, 96), (8, 2), (64, 0), (1024, 96), (1 << 30, 0), (1 << 30, 7), (1 << 30, 256)])
+def test_loop_threshold_sweep_same_schedule(gd, hi, small):
     # whatever share of the steps the loop takes (hi = largest active set it accepts), the schedule is the same
     w = W.config(1)
     t_end = 2.0 ** -5
@@ -367,6 +367,7 @@ def test_loop_threshold_sweep_same_schedule(gd, hi):
     ref.run_until(t_end)
     h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
     h.set_option("loop_max_nact", hi)
+    h.set_option("loop_small_nact", small)
     steps, psteps = h.run_until(t_end)
     assert h.t == ref.t == t_end and steps == ref.block_steps and psteps == ref.particle_steps
     a, b = h.state_host(), ref.state_host()
