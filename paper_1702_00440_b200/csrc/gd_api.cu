@@ -180,6 +180,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->ipar_small_max_nact = 2048;
     c->loop_max_nact = (int64_t)1 << 40;      // every step the scratch allows
     c->loop_small_nact = 96;
+    c->loop_state_opt = 1;
     c->stream = (cudaStream_t)stream;
     gd_carve(&c->d, ws, c->np, c->pcap);
     int dev = 0;
@@ -261,9 +262,10 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
     if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "ipar_small_max_nact")) { c->ipar_small_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "use_graph")) { c->use_graph = value != 0.0; return GD_OK; }
-    if (!strcmp(key, "loop_max_nact") || !strcmp(key, "loop_small_nact")) {
+    if (!strcmp(key, "loop_max_nact") || !strcmp(key, "loop_small_nact") || !strcmp(key, "loop_state_smem")) {
         if (!strcmp(key, "loop_max_nact")) c->loop_max_nact = (int64_t)value;
-        else c->loop_small_nact = (int64_t)value;
+        else if (!strcmp(key, "loop_small_nact")) c->loop_small_nact = (int64_t)value;
+        else c->loop_state_opt = value != 0.0;
         gd_graph_drop(c);
         return gdk_loop_setup(c);
     }
@@ -565,7 +567,7 @@ extern "C" int gd_get_profile(gd_ctx *c, double *prof_host)
 extern "C" int gd_get_loop_profile(gd_ctx *c, int64_t *out_host)
 {
     if (!c || !out_host) return GD_EINVAL;
-    GD_CUDA(c, cudaMemcpyAsync(out_host, c->d.lp_ctl + 2, 8 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaMemcpyAsync(out_host, c->d.lp_ctl + 2, 14 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
     GD_CUDA(c, cudaStreamSynchronize(c->stream));
     return GD_OK;
 }

@@ -83,8 +83,9 @@ struct gd_ctx {
     gd_ctrl *h_ctrl;                     // pinned host mirror of d.ctrl
     int use_graph;
     int64_t loop_max_nact;               // option: largest active set the persistent loop takes (0 = loop off)
+    int loop_state_opt;                  // option: keep the own state resident in shared memory when it fits
     int64_t loop_small_nact;             // option: active sets up to this size use the lanes-over-sources mapping
-    int loop_grid, loop_S, loop_hi, loop_cap;   // geometry of k_block_loop (loop_grid = 0: not usable)
+    int loop_grid, loop_S, loop_hi, loop_cap, loop_state;   // geometry of k_block_loop (loop_grid = 0: not usable)
     size_t loop_smem;
     int64_t graph_nodes;                 // kernel nodes in step_graph
     int sm_count;

@@ -18,7 +18,7 @@ __device__ __forceinline__ gd_pred gd_predict_record(const double4 &xm, const do
 {
     double D = gd_sub(t, vt.w);
     double DD = gd_mul(D, D);
-    double D2 = gd_div(DD, 2.0);
+    double D2 = gd_mul(DD, 0.5);                              // = DD / 2 exactly
     double D3 = gd_div(gd_mul(DD, D), 6.0);
 #define GD_PX(x0, v0, a0, j0) gd_add(gd_add(gd_add((x0), gd_mul((v0), D)), gd_mul((a0), D2)), gd_mul((j0), D3))
 #define GD_PV(v0, a0, j0) gd_add(gd_add((v0), gd_mul((a0), D)), gd_mul((j0), D2))
@@ -36,8 +36,10 @@ __device__ __forceinline__ gd_pred gd_predict_record(const double4 &xm, const do
 
 // ---- corrector, one Cartesian component ----------------------------------------------------------------------
 struct gd_corr1 { double xnew, vnew, a2e, a3; };
-struct gd_hpow { double h, h2, h3, h4, h5; };
+struct gd_hpow { double h, h2, h3, h4, h5, ih2, ih3; bool pow2; };
 
+// Block steps are powers of two (R5), so x / h^2 and x / h^3 are exact scalings: they are done as
+// multiplications by 2^(2k), 2^(3k), bit for bit the quotient (any other h keeps the division).
 __device__ __forceinline__ gd_hpow gd_step_powers(double h)
 {
     gd_hpow p;
@@ -46,6 +48,12 @@ __device__ __forceinline__ gd_hpow gd_step_powers(double h)
     p.h3 = gd_mul(p.h2, h);
     p.h4 = gd_mul(p.h2, p.h2);
     p.h5 = gd_mul(p.h4, h);
+    const long long bits = __double_as_longlong(h);
+    const long long ef = (bits >> 52) & 0x7ff;
+    p.pow2 = bits > 0 && (bits & 0xfffffffffffffLL) == 0 && ef >= 1023 - 300 && ef <= 1023 + 300;
+    const double ih = __longlong_as_double((2046LL - ef) << 52);
+    p.ih2 = gd_mul(ih, ih);
+    p.ih3 = gd_mul(p.ih2, ih);
     return p;
 }
 
@@ -54,9 +62,11 @@ __device__ __forceinline__ gd_corr1 gd_correct_component(double xp, double vp, d
     const double h = p.h;
     double da = gd_sub(a0, a1);
     // a2 = (-6 (a0 - a1) - h (4 j0 + 2 j1)) / h^2
-    double a2 = gd_div(gd_sub(gd_mul(-6.0, da), gd_mul(h, gd_add(gd_mul(4.0, j0), gd_mul(2.0, j1)))), p.h2);
+    const double n2 = gd_sub(gd_mul(-6.0, da), gd_mul(h, gd_add(gd_mul(4.0, j0), gd_mul(2.0, j1))));
+    double a2 = p.pow2 ? gd_mul(n2, p.ih2) : gd_div(n2, p.h2);
     // a3 = (12 (a0 - a1) + 6 h (j0 + j1)) / h^3
-    double a3 = gd_div(gd_add(gd_mul(12.0, da), gd_mul(gd_mul(6.0, h), gd_add(j0, j1))), p.h3);
+    const double n3 = gd_add(gd_mul(12.0, da), gd_mul(gd_mul(6.0, h), gd_add(j0, j1)));
+    double a3 = p.pow2 ? gd_mul(n3, p.ih3) : gd_div(n3, p.h3);
     gd_corr1 r;
     // x = xp + a2 h^4/24 + a3 h^5/120 ;  v = vp + a2 h^3/6 + a3 h^4/24
     r.xnew = gd_add(gd_add(xp, gd_div(gd_mul(a2, p.h4), 24.0)), gd_div(gd_mul(a3, p.h5), 120.0));

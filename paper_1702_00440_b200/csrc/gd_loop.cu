@@ -40,6 +40,7 @@ struct gd_largs {
     int hi;                          // largest active set the loop takes
     int cap;                         // row length of the partial sums: partial[c][comp][cap]
     int small_hi;                    // n_act <= small_hi: lanes over sources; above: lanes over sinks
+    int state;                       // != 0: the own state is resident in shared memory
     double eps2, eta, dt_min, dt_max;
     int halving_mode;
 };
@@ -141,18 +142,26 @@ struct gd_lsm {
     double *wmin;                    // [GD_LP_WARPS]
     int *wcnt;                       // [GD_LP_WARPS + 1]
     unsigned int *hist;              // [64] particle steps per level, [64..65] diagnostics
+    double4 *xm, *vt, *ad, *jk;      // [S] own state (only when it fits: `state` != 0; global memory is written through)
 };
 
-__host__ __device__ inline size_t gd_lsm_bytes(int S)
+__host__ __device__ inline size_t gd_lsm_bytes(int S, int state)
 {
-    return (size_t)S * (16 * 3 + 8 + 8 + 4) + GD_LP_WARPS * 6 * 32 * 8 + GD_LP_WARPS * 8 + GD_LP_MAX_SMALL * 4 +
+    return (size_t)S * (16 * 3 + 8 + 8 + 4 + (state ? 128 : 0)) + GD_LP_WARPS * 6 * 32 * 8 + GD_LP_WARPS * 8 + GD_LP_MAX_SMALL * 4 +
            (GD_LP_MAX_GRID + 1) * 4 + (GD_LP_WARPS + 1) * 4 + 66 * 4 + 64;
 }
 
-__device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S)
+__device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S, int state)
 {
     gd_lsm s;
     unsigned char *p = base;
+    s.xm = s.vt = s.ad = s.jk = nullptr;
+    if (state) {
+        s.xm = (double4 *)p; p += (size_t)S * 32;
+        s.vt = (double4 *)p; p += (size_t)S * 32;
+        s.ad = (double4 *)p; p += (size_t)S * 32;
+        s.jk = (double4 *)p; p += (size_t)S * 32;
+    }
     s.pxy = (double2 *)p; p += (size_t)S * 16;
     s.pzm = (double2 *)p; p += (size_t)S * 16;
     s.vxy = (double2 *)p; p += (size_t)S * 16;
@@ -167,6 +176,12 @@ __device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S)
     s.hist = (unsigned int *)p;
     return s;
 }
+
+// own state of local particle p (global index i): shared memory when resident, else global memory (owner-only data)
+#define GD_LP_XM(p, i) (sm.xm ? sm.xm[p] : d.xm[i])
+#define GD_LP_VT(p, i) (sm.xm ? sm.vt[p] : d.vt[i])
+#define GD_LP_AD(p, i) (sm.xm ? sm.ad[p] : d.ad[i])
+#define GD_LP_JK(p, i) (sm.xm ? sm.jk[p] : d.jk[i])
 
 // ---- [publish]: L_c, the candidates of this CTA (ascending), their records predicted to L_c ------------------------------
 // rec row r = two double4: {xp, yp, zp, particle index (as an integer in a double)}, {vxp, vyp, vzp, 0}
@@ -203,8 +218,8 @@ __device__ __forceinline__ int gd_publish(const gd_dev &d, const gd_lsm &sm, int
     }
     const int cnt = base;
     for (int k = tid; k < cnt; k += GD_LP_THREADS) {
-        const int i = p0 + sm.lact[k];
-        const double4 xm = d.xm[i], vt = d.vt[i], ad = d.ad[i], jk = d.jk[i];
+        const int p = sm.lact[k], i = p0 + p;
+        const double4 xm = GD_LP_XM(p, i), vt = GD_LP_VT(p, i), ad = GD_LP_AD(p, i), jk = GD_LP_JK(p, i);
         const gd_pred q = gd_predict_record(xm, vt, ad, jk, L);
         double4 *row = d.lp_rec + 2 * (size_t)(p0 + k);
         row[0] = make_double4(q.x, q.y, q.z, (double)i);
@@ -406,10 +421,10 @@ __device__ __forceinline__ void gd_lp_commit(const gd_dev &d, const gd_lsm &sm, 
     if (r.flags & 2) atomicAdd(&sm.hist[65], 1u);
     const int lvl = gd_step_level(h);
     if (lvl >= 0 && lvl < 64) atomicAdd(&sm.hist[lvl], 1u);
-    d.xm[i] = make_double4(r.x, r.y, r.z, m);
-    d.vt[i] = make_double4(r.vx, r.vy, r.vz, t_next);
-    d.ad[i] = make_double4(a1[0], a1[1], a1[2], r.dt);
-    d.jk[i] = make_double4(j1[0], j1[1], j1[2], 0.0);
+    const double4 xm = make_double4(r.x, r.y, r.z, m), vt = make_double4(r.vx, r.vy, r.vz, t_next);
+    const double4 ad = make_double4(a1[0], a1[1], a1[2], r.dt), jk = make_double4(j1[0], j1[1], j1[2], 0.0);
+    d.xm[i] = xm; d.vt[i] = vt; d.ad[i] = ad; d.jk[i] = jk;
+    if (sm.xm) { sm.xm[p] = xm; sm.vt[p] = vt; sm.ad[p] = ad; sm.jk[p] = jk; }
     const double tn = t_next + r.dt;                         // exact (dyadic)
     d.tnext[i] = tn;
     sm.ts[p] = tn;
@@ -421,19 +436,35 @@ __device__ __forceinline__ void gd_lp_commit(const gd_dev &d, const gd_lsm &sm, 
 __device__ __forceinline__ void gd_lp_correct_warp(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, int G, int p0, int pos, int p,
                                                    double t_next, int lane)
 {
+    const long long c0 = clock64();
     const int i = p0 + p;
-    const double4 ad = d.ad[i], jk = d.jk[i];
+    const double4 ad = GD_LP_AD(p, i), jk = GD_LP_JK(p, i);
     double s[6] = {0, 0, 0, 0, 0, 0};
-    for (int c = lane; c < G; c += 32) {
-        const double *row = d.partial + (size_t)c * 6 * la.cap + pos;
+    {   // all loads of this lane in flight at once (G <= GD_LP_MAX_GRID = 8 x 32), then added in ascending c
+        double v[GD_LP_MAX_GRID / 32][6];
 #pragma unroll
-        for (int k = 0; k < 6; ++k) s[k] += __ldcg(row + (size_t)k * la.cap);
+        for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
+            const int c = lane + 32 * u;
+            const double *row = d.partial + (size_t)(c < G ? c : lane) * 6 * la.cap + pos;
+            if (32 * u < G) {
+#pragma unroll
+                for (int k = 0; k < 6; ++k) v[u][k] = __ldcg(row + (size_t)k * la.cap);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
+            if (lane + 32 * u < G) {
+#pragma unroll
+                for (int k = 0; k < 6; ++k) s[k] += v[u][k];
+            }
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
         for (int k = 0; k < 6; ++k) s[k] += __shfl_xor_sync(GD_FULL, s[k], o);
     }
+    const long long c1 = clock64();
     const double2 pxy = sm.pxy[p], pzm = sm.pzm[p], pvxy = sm.vxy[p];
     const double pvz = sm.vz[p];
     const int comp = lane < 2 ? lane : 2;
@@ -454,9 +485,16 @@ __device__ __forceinline__ void gd_lp_correct_warp(const gd_dev &d, const gd_lsm
     const double na1 = gd_norm3(s[0], s[1], s[2]), nj1 = gd_norm3(s[3], s[4], s[5]);
     const double na2 = gd_norm3(a2x, a2y, a2z), na3 = gd_norm3(a3x, a3y, a3z);
     r.dt = gd_new_step(na1, nj1, na2, na3, h, t_next, la.eta, la.dt_min, la.dt_max, la.halving_mode, r.flags);
+    const long long c2 = clock64();
     if (lane == 0) {
         const double a1v[3] = {s[0], s[1], s[2]}, j1v[3] = {s[3], s[4], s[5]};
         gd_lp_commit(d, sm, i, p, pzm.y, r, a1v, j1v, h, t_next);
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            const long long c3 = clock64();
+            d.lp_ctl[13] += (unsigned long long)(c1 - c0);
+            d.lp_ctl[14] += (unsigned long long)(c2 - c1);
+            d.lp_ctl[15] += (unsigned long long)(c3 - c2);
+        }
     }
 }
 
@@ -465,14 +503,26 @@ __device__ __forceinline__ void gd_lp_correct_thread(const gd_dev &d, const gd_l
                                                      double t_next)
 {
     const int i = p0 + p;
-    const double4 ad = d.ad[i], jk = d.jk[i];
+    const double4 ad = GD_LP_AD(p, i), jk = GD_LP_JK(p, i);
     double s[6] = {0, 0, 0, 0, 0, 0};
     const double *row = d.partial + pos;
     const size_t cs = (size_t)6 * la.cap;
-#pragma unroll 4
-    for (int c = 0; c < G; ++c) {
+    // batches of 16 CTAs: 96 loads in flight, then added in ascending c
+    for (int c0 = 0; c0 < G; c0 += 16) {
+        double v[16][6];
 #pragma unroll
-        for (int k = 0; k < 6; ++k) s[k] += __ldcg(row + (size_t)c * cs + (size_t)k * la.cap);
+        for (int u = 0; u < 16; ++u) {
+            const int c = min(c0 + u, G - 1);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) v[u][k] = __ldcg(row + (size_t)c * cs + (size_t)k * la.cap);
+        }
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            if (c0 + u < G) {
+#pragma unroll
+                for (int k = 0; k < 6; ++k) s[k] += v[u][k];
+            }
+        }
     }
     const double2 pxy = sm.pxy[p], pzm = sm.pzm[p], pvxy = sm.vxy[p];
     const double pvz = sm.vz[p];
@@ -492,7 +542,7 @@ k_block_loop(gd_dev d, gd_largs la)
     extern __shared__ __align__(16) unsigned char gd_lp_smem[];
     gd_ctrl *ct = d.ctrl;
     if (ct->finished) return;                                // nobody writes ct before the first barrier
-    const gd_lsm sm = gd_lsm_carve(gd_lp_smem, la.S);
+    const gd_lsm sm = gd_lsm_carve(gd_lp_smem, la.S, la.state);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = gridDim.x, me = blockIdx.x;
     const int p0 = gd_slice_begin(me, la.n, G);
@@ -510,6 +560,7 @@ k_block_loop(gd_dev d, gd_largs la)
     for (int p = tid; p < rounds * 32; p += GD_LP_THREADS) {
         if (p < cnt_own) {
             sm.ts[p] = d.tnext[p0 + p];
+            if (sm.xm) { sm.xm[p] = d.xm[p0 + p]; sm.vt[p] = d.vt[p0 + p]; sm.ad[p] = d.ad[p0 + p]; sm.jk[p] = d.jk[p0 + p]; }
         } else {                                             // zero-mass padding of the last source round
             sm.pxy[p] = make_double2(0.0, 0.0);
             sm.pzm[p] = make_double2(0.0, 0.0);
@@ -526,7 +577,7 @@ k_block_loop(gd_dev d, gd_largs la)
     gd_bar_wait(bar, target);
 
     bool fin = false;
-    unsigned long long tr[4] = {0, 0, 0, 0}, g0 = gd_gtime(), g1;   // CTA 0's view: ns in [force], barrier, [correct], barrier
+    unsigned long long tr[4] = {0, 0, 0, 0}, own[3] = {0, 0, 0}, g0 = gd_gtime(), g1;   // CTA 0's view: ns in [force], barrier, [correct], barrier
     const unsigned long long g_begin = g0;
     for (;;) {
         if (t_cur >= t_end || (max_steps >= 0 && steps >= max_steps)) { fin = true; break; }
@@ -560,7 +611,7 @@ k_block_loop(gd_dev d, gd_largs la)
         // own slice predicted to t+
         for (int p = tid; p < cnt_own; p += GD_LP_THREADS) {
             const int i = p0 + p;
-            const double4 xm = d.xm[i], vt = d.vt[i], ad = d.ad[i], jk = d.jk[i];
+            const double4 xm = GD_LP_XM(p, i), vt = GD_LP_VT(p, i), ad = GD_LP_AD(p, i), jk = GD_LP_JK(p, i);
             const gd_pred q = gd_predict_record(xm, vt, ad, jk, t_next);
             sm.pxy[p] = make_double2(q.x, q.y);
             sm.pzm[p] = make_double2(q.z, xm.w);
@@ -578,14 +629,18 @@ k_block_loop(gd_dev d, gd_largs la)
         // ---- [correct] + [publish] ----
         const bool contributing = (L_me == t_next) && cnt_me > 0;
         if (contributing) {
+            const unsigned long long o0 = gd_gtime();
             const int pre = sm.spre[me];
-            if (small) {
+            // few own active particles: a warp each (lanes over the CTAs' partial sums); many: a thread each
+            if (cnt_me <= 2 * GD_LP_WARPS) {
                 for (int k = warp; k < cnt_me; k += GD_LP_WARPS) gd_lp_correct_warp(d, sm, la, G, p0, pre + k, sm.lact[k], t_next, lane);
             } else {
                 for (int k = tid; k < cnt_me; k += GD_LP_THREADS) gd_lp_correct_thread(d, sm, la, G, p0, pre + k, sm.lact[k], t_next);
             }
             __syncthreads();
+            const unsigned long long o1 = gd_gtime();
             cnt_me = gd_publish(d, sm, me, p0, cnt_own, &L_me);
+            own[0] += 1; own[1] += o1 - o0; own[2] += gd_gtime() - o1;
         }
         t_cur = t_next;
         steps += 1;
@@ -612,6 +667,7 @@ k_block_loop(gd_dev d, gd_largs la)
         d.lp_ctl[4] += gd_gtime() - g_begin;
         for (int k = 0; k < 4; ++k) d.lp_ctl[5 + k] += tr[k];
         d.lp_ctl[9] += 1ull;
+        for (int k = 0; k < 3; ++k) d.lp_ctl[10 + k] += own[k];   // CTA 0 as an owner: steps, ns correcting, ns publishing
     }
 }
 
@@ -634,7 +690,9 @@ int gdk_loop_setup(gd_ctx *c)
     GD_CUDA(c, cudaGetDevice(&dev));
     GD_CUDA(c, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     GD_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
-    const size_t bytes = gd_lsm_bytes((int)S);
+    int state = c->loop_state_opt ? 1 : 0;
+    size_t bytes = gd_lsm_bytes((int)S, state);
+    if (bytes > (size_t)max_smem) { state = 0; bytes = gd_lsm_bytes((int)S, 0); }
     if (!coop || bytes > (size_t)max_smem) return 0;
     GD_CUDA(c, cudaFuncSetAttribute(k_block_loop<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     GD_CUDA(c, cudaFuncSetAttribute(k_block_loop<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
@@ -646,6 +704,7 @@ int gdk_loop_setup(gd_ctx *c)
     c->loop_hi = (int)hi;
     c->loop_cap = (int)cap;
     c->loop_smem = bytes;
+    c->loop_state = state;
     return 0;
 }
 
@@ -658,6 +717,7 @@ int gdk_loop(gd_ctx *c)
     la.S = c->loop_S;
     la.hi = c->loop_hi;
     la.cap = c->loop_cap;
+    la.state = c->loop_state;
     int64_t sh = c->loop_small_nact < GD_LP_MAX_SMALL ? c->loop_small_nact : GD_LP_MAX_SMALL;
     la.small_hi = (int)(sh < 0 ? 0 : sh);
     la.eps2 = c->eps2;
