@@ -38,7 +38,7 @@ struct gd_largs {
     int n;                           // particles; CTA c owns [c n / G, (c + 1) n / G)
     int S;                           // slice capacity in shared memory (multiple of 32)
     int hi;                          // largest active set the loop takes
-    int cap;                         // row length of the partial sums: partial[c][comp][cap]
+    int cap;                         // rows of 6 partial sums per CTA: partial[c][cap][6]
     int small_hi;                    // n_act <= small_hi: lanes over sources; above: lanes over sinks
     int state;                       // != 0: the own state is resident in shared memory
     double eps2, eta, dt_min, dt_max;
@@ -270,11 +270,10 @@ __device__ __forceinline__ void gd_lp_item(const gd_dev &d, const gd_lsm &sm, in
     }
 }
 
-// element e = b * 6 + comp of the block starting at position pos -> partial[me][comp][pos + b]
+// element e = b * 6 + comp of the block starting at position pos -> partial[me][pos + b][comp]
 __device__ __forceinline__ void gd_lp_put(double *out, int cap, int pos, int e, double val)
 {
-    const int b = e / 6, comp = e - 6 * b;
-    out[(size_t)comp * cap + pos + b] = val;
+    out[(size_t)pos * 6 + e] = val;
 }
 
 // One work item = a register block of sinks: items 0 .. n4 - 1 hold 4 sinks, the n_act % 4 last ones hold 1.
@@ -385,8 +384,8 @@ __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &s
             const gd_src si = gd_lp_load_sink(d, gd_lp_row_of(sm, min(pos, n_act - 1), la.n, G));
             const gd_acc a = gd_lp_tile<EPS0>(sm, si, 0, cnt_own, la.eps2);
             if (pos < n_act) {
-                out[pos] = a.ax; out[(size_t)la.cap + pos] = a.ay; out[(size_t)2 * la.cap + pos] = a.az;
-                out[(size_t)3 * la.cap + pos] = a.jx; out[(size_t)4 * la.cap + pos] = a.jy; out[(size_t)5 * la.cap + pos] = a.jz;
+                double2 *o = reinterpret_cast<double2 *>(out + (size_t)pos * 6);
+                o[0] = make_double2(a.ax, a.ay); o[1] = make_double2(a.az, a.jx); o[2] = make_double2(a.jy, a.jz);
             }
         }
         return;
@@ -408,7 +407,7 @@ __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &s
         for (int comp = 0; comp < 6; ++comp) {
             double s = sm.red[warp * 192 + comp * 32 + lane];
             for (int c = 1; c < nsplit; ++c) s += sm.red[(warp + c) * 192 + comp * 32 + lane];
-            out[(size_t)comp * la.cap + pos] = s;
+            out[(size_t)pos * 6 + comp] = s;
         }
     }
 }
@@ -440,24 +439,10 @@ __device__ __forceinline__ void gd_lp_correct_warp(const gd_dev &d, const gd_lsm
     const int i = p0 + p;
     const double4 ad = GD_LP_AD(p, i), jk = GD_LP_JK(p, i);
     double s[6] = {0, 0, 0, 0, 0, 0};
-    {   // all loads of this lane in flight at once (G <= GD_LP_MAX_GRID = 8 x 32), then added in ascending c
-        double v[GD_LP_MAX_GRID / 32][6];
-#pragma unroll
-        for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
-            const int c = lane + 32 * u;
-            const double *row = d.partial + (size_t)(c < G ? c : lane) * 6 * la.cap + pos;
-            if (32 * u < G) {
-#pragma unroll
-                for (int k = 0; k < 6; ++k) v[u][k] = __ldcg(row + (size_t)k * la.cap);
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
-            if (lane + 32 * u < G) {
-#pragma unroll
-                for (int k = 0; k < 6; ++k) s[k] += v[u][k];
-            }
-        }
+    for (int c = lane; c < G; c += 32) {
+        const double2 *row = reinterpret_cast<const double2 *>(d.partial + ((size_t)c * la.cap + pos) * 6);
+        const double2 u0 = __ldcg(row), u1 = __ldcg(row + 1), u2 = __ldcg(row + 2);
+        s[0] += u0.x; s[1] += u0.y; s[2] += u1.x; s[3] += u1.y; s[4] += u2.x; s[5] += u2.y;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -505,22 +490,21 @@ __device__ __forceinline__ void gd_lp_correct_thread(const gd_dev &d, const gd_l
     const int i = p0 + p;
     const double4 ad = GD_LP_AD(p, i), jk = GD_LP_JK(p, i);
     double s[6] = {0, 0, 0, 0, 0, 0};
-    const double *row = d.partial + pos;
-    const size_t cs = (size_t)6 * la.cap;
-    // batches of 16 CTAs: 96 loads in flight, then added in ascending c
+    const double2 *row = reinterpret_cast<const double2 *>(d.partial + (size_t)pos * 6);
+    const size_t cs = (size_t)3 * la.cap;                    // double2 per CTA
+    // batches of 16 CTAs: 48 loads in flight, then added in ascending c
     for (int c0 = 0; c0 < G; c0 += 16) {
-        double v[16][6];
+        double2 v[16][3];
 #pragma unroll
         for (int u = 0; u < 16; ++u) {
             const int c = min(c0 + u, G - 1);
 #pragma unroll
-            for (int k = 0; k < 6; ++k) v[u][k] = __ldcg(row + (size_t)c * cs + (size_t)k * la.cap);
+            for (int k = 0; k < 3; ++k) v[u][k] = __ldcg(row + (size_t)c * cs + k);
         }
 #pragma unroll
         for (int u = 0; u < 16; ++u) {
             if (c0 + u < G) {
-#pragma unroll
-                for (int k = 0; k < 6; ++k) s[k] += v[u][k];
+                s[0] += v[u][0].x; s[1] += v[u][0].y; s[2] += v[u][1].x; s[3] += v[u][1].y; s[4] += v[u][2].x; s[5] += v[u][2].y;
             }
         }
     }
