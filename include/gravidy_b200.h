@@ -168,8 +168,10 @@ GD_API int gd_get_loop_profile(gd_ctx *ctx, int64_t *out_host);
 
 /* Optional CUDA-event timing of the force launches, switched on with gd_set_option(ctx, "profile", 1): every
  * gd_force_jerk issued afterwards is bracketed by two events on the context's stream (the all-active evaluation
- * inside gd_init runs before the option can be set and is not timed).  prof_host[12] receives, for kind k = 0
- * (i-parallel kernel, 256-sink tiles), 1 (j-split kernel), 2 (i-parallel kernel, 32-sink tiles):
+ * inside gd_init runs before the option can be set and is not timed); gd_step / gd_run_until then launch the
+ * persistent block-step loop directly instead of replaying the graph, each launch bracketed the same way.
+ * prof_host[16] receives, for kind k = 0 (i-parallel kernel, 256-sink tiles), 1 (j-split kernel), 2 (i-parallel
+ * kernel, 32-sink tiles), 3 (k_block_loop: pairs = particle steps taken inside the loop x n):
  *   prof[4k] launches timed, prof[4k+1] sum of durations in ms, prof[4k+2] sum of pair interactions (n_act * n),
  *   prof[4k+3] sum of squared durations (ms^2).  Synchronises on the last recorded event. */
 GD_API int gd_get_profile(gd_ctx *ctx, double *prof_host);

@@ -298,10 +298,10 @@ class Hermite:
 
     def profile(self) -> dict:
         """Event-timed force launches since the "profile" option was set: per kernel launches, ms, pairs."""
-        p = np.zeros(12)
+        p = np.zeros(16)
         self._check(self._lib.gd_get_profile(self._h, p.ctypes.data))
         return {k: {"launches": int(p[4 * i]), "ms": float(p[4 * i + 1]), "pairs": float(p[4 * i + 2]),
-                    "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit", "ipar_small"))}
+                    "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit", "ipar_small", "loop"))}
 
     def loop_profile(self) -> dict:
         o = np.zeros(14, dtype=np.int64)

@@ -452,12 +452,51 @@ static int gd_run_graph(gd_ctx *c, double t_end, int64_t max_steps, int64_t *ste
     return GD_OK;
 }
 
+// "profile" option with the persistent loop available: the same sequence as the graph (loop, then the stage kernels
+// for the one step it left), launched directly so that every loop launch is bracketed by two events (kind 3).
+static int gd_run_profiled(gd_ctx *c, double t_end, int64_t max_steps, int64_t *steps_out, int64_t *psteps_out)
+{
+    gd_ctrl *up = c->h_ctrl, *down = c->h_ctrl + 1;
+    up->t_end = t_end;
+    up->t = c->t;
+    up->max_steps = max_steps;
+    up->steps = up->psteps = up->finished = 0;
+    unsigned long long lp0 = 0, lp1 = 0;
+    GD_CUDA(c, cudaMemcpyAsync(c->d.ctrl, up, sizeof(gd_ctrl), cudaMemcpyHostToDevice, c->stream));
+    GD_CUDA(c, cudaMemcpyAsync(&lp0, c->d.lp_ctl + 2, 8, cudaMemcpyDeviceToHost, c->stream));
+    for (;;) {
+        const int slot = gd_prof_begin(c);
+        int rc = gdk_loop(c);
+        gd_prof_end(c, slot, 3, 0.0);
+        if (!rc) rc = gdk_next_block(c, true);
+        if (!rc) rc = gdk_predict(c, 0.0, true);
+        if (!rc) rc = gdk_force_dev(c);
+        if (!rc) rc = gdk_correct(c, 0.0, true);
+        if (rc) return rc;
+        GD_CUDA(c, cudaMemcpyAsync(down, c->d.ctrl, sizeof(gd_ctrl), cudaMemcpyDeviceToHost, c->stream));
+        GD_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (down->finished) break;
+    }
+    GD_CUDA(c, cudaMemcpyAsync(&lp1, c->d.lp_ctl + 2, 8, cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->prof[4 * 3 + 2] += (double)(lp1 - lp0) * (double)c->n;         // pairs evaluated inside the loop
+    c->t = down->t;
+    c->block_steps += down->steps;
+    c->particle_steps += down->psteps;
+    c->have_block = c->have_force = c->have_pred = false;
+    if (steps_out) *steps_out = down->steps;
+    if (psteps_out) *psteps_out = down->psteps;
+    return GD_OK;
+}
+
 extern "C" int gd_step(gd_ctx *c, int64_t n_steps, int64_t *particle_steps_host)
 {
     if (!c) return GD_EINVAL;
     if (c->lvl_min > c->lvl_max) return gd_fail(c, GD_ESTATE, "gd_step: dt_level_min > dt_level_max");
     if (c->use_graph && !c->profile && n_steps >= GD_GRAPH_STEPS / 2)
         return gd_run_graph(c, INFINITY, n_steps, nullptr, particle_steps_host);
+    if (c->use_graph && c->profile && c->loop_grid > 0 && n_steps >= GD_GRAPH_STEPS / 2)
+        return gd_run_profiled(c, INFINITY, n_steps, nullptr, particle_steps_host);
     int64_t before = c->particle_steps;
     for (int64_t s = 0; s < n_steps; ++s) {
         int rc = gd_one_step(c);
@@ -475,6 +514,8 @@ extern "C" int gd_run_until(gd_ctx *c, double t_end, int64_t max_steps, int64_t 
     if (c->lvl_min > c->lvl_max) return gd_fail(c, GD_ESTATE, "gd_run_until: dt_level_min > dt_level_max");
     if (c->use_graph && !c->profile && c->t < t_end && max_steps != 0)
         return gd_run_graph(c, t_end, max_steps, steps_host, particle_steps_host);
+    if (c->use_graph && c->profile && c->loop_grid > 0 && c->t < t_end && max_steps != 0)
+        return gd_run_profiled(c, t_end, max_steps, steps_host, particle_steps_host);
     int64_t before = c->particle_steps, steps = 0;
     while (c->t < t_end && (max_steps < 0 || steps < max_steps)) {
         int rc = gd_one_step(c);

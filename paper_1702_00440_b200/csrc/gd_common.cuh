@@ -96,7 +96,7 @@ struct gd_ctx {
     int ev_kind[GD_PROF_POOL];
     int ev_pending;
     bool ev_created;
-    double prof[12];             // per kind k = 0 (i-parallel), 1 (j-split), 2 (other stages): {launches, ms, pairs, ms^2}
+    double prof[16];             // per kind k = 0 (i-parallel L), 1 (j-split), 2 (i-parallel S), 3 (block-step loop): {launches, ms, pairs, ms^2}
     char err[512];
 };
 
