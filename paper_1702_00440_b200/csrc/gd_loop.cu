@@ -70,18 +70,22 @@ __device__ __forceinline__ void gd_bar_wait(unsigned long long *bar, unsigned lo
     __syncthreads();
 }
 
+// device global timer, read by thread 0 of CTA 0 only (the read is slow); 0 elsewhere
 __device__ __forceinline__ unsigned long long gd_gtime()
 {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    unsigned long long t = 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
     return t;
 }
 
+// warp minimum of non-negative doubles (times, +inf): their order is the order of their bit patterns, so two
+// integer warp reductions (REDUX) do it -- high words first, then the low words of the lanes that tie
 __device__ __forceinline__ double gd_warp_min_d(double v)
 {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(GD_FULL, v, o));
-    return v;
+    const unsigned int hi = (unsigned int)__double2hiint(v), lo = (unsigned int)__double2loint(v);
+    const unsigned int mh = __reduce_min_sync(GD_FULL, hi);
+    const unsigned int ml = __reduce_min_sync(GD_FULL, hi == mh ? lo : 0xffffffffu);
+    return __hiloint2double((int)mh, (int)ml);
 }
 
 // ---- fixed-tree warp reduce-scatter ---------------------------------------------------------------------------------
@@ -361,6 +365,21 @@ __device__ __forceinline__ gd_acc gd_lp_tile(const gd_lsm &sm, const gd_src &si,
     return a0;
 }
 
+// wide tiles: BI sinks per lane (positions pos0 + 32 b + lane) against the whole slice, one accumulator set per sink
+template <int BI, bool EPS0>
+__device__ __forceinline__ void gd_lp_tile_wide(const gd_lsm &sm, const gd_src (&si)[BI], int cnt, double eps2, gd_acc (&acc)[BI])
+{
+#pragma unroll
+    for (int b = 0; b < BI; ++b) acc[b] = gd_acc{0, 0, 0, 0, 0, 0};
+#pragma unroll 2
+    for (int j = 0; j < cnt; ++j) {
+        const double2 xy = sm.pxy[j], zm = sm.pzm[j], vxy = sm.vxy[j];
+        const gd_src sj{xy.x, xy.y, zm.x, zm.y, vxy.x, vxy.y, sm.vz[j]};
+#pragma unroll
+        for (int b = 0; b < BI; ++b) gd_pair<EPS0>(si[b], sj, eps2, acc[b]);
+    }
+}
+
 // position in the active list -> row of rec: CTA c with spre[c] <= pos < spre[c + 1] (segments of empty CTAs have
 // zero width), row = first row of c's segment + offset
 __device__ __forceinline__ int gd_lp_row_of(const gd_lsm &sm, int pos, int n, int G)
@@ -373,9 +392,36 @@ __device__ __forceinline__ int gd_lp_row_of(const gd_lsm &sm, int pos, int n, in
     return gd_slice_begin(lo, n, G) + (pos - sm.spre[lo]);
 }
 
+template <int BI, bool EPS0>
+__device__ __forceinline__ void gd_lp_force_wide(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int G, int n_act, int cnt_own)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int tiles = (n_act + 32 * BI - 1) / (32 * BI);
+    for (int tile = warp; tile < tiles; tile += GD_LP_WARPS) {
+        gd_src si[BI];
+        gd_acc acc[BI];
+#pragma unroll
+        for (int b = 0; b < BI; ++b)
+            si[b] = gd_lp_load_sink(d, gd_lp_row_of(sm, min(tile * 32 * BI + 32 * b + lane, n_act - 1), la.n, G));
+        gd_lp_tile_wide<BI, EPS0>(sm, si, cnt_own, la.eps2, acc);
+#pragma unroll
+        for (int b = 0; b < BI; ++b) {
+            const int pos = tile * 32 * BI + 32 * b + lane;
+            if (pos < n_act) {
+                double2 *o = reinterpret_cast<double2 *>(out + (size_t)pos * 6);
+                o[0] = make_double2(acc[b].ax, acc[b].ay); o[1] = make_double2(acc[b].az, acc[b].jx); o[2] = make_double2(acc[b].jy, acc[b].jz);
+            }
+        }
+    }
+}
+
 template <bool EPS0>
 __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int G, int n_act, int cnt_own)
 {
+    // enough sinks for every warp to hold several per lane: more independent pair chains per warp (the FP64 pipe
+    // needs ~8 per scheduler to stay busy), fewer shared-memory reads per pair
+    if (n_act >= 3 * 128 * GD_LP_WARPS) { gd_lp_force_wide<4, EPS0>(d, sm, la, out, G, n_act, cnt_own); return; }
+    if (n_act >= 2 * 64 * GD_LP_WARPS) { gd_lp_force_wide<2, EPS0>(d, sm, la, out, G, n_act, cnt_own); return; }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tiles = (n_act + 31) >> 5;
     if (tiles >= GD_LP_WARPS) {
