@@ -38,7 +38,7 @@ struct gd_largs {
     int n;                           // particles; CTA c owns [c n / G, (c + 1) n / G)
     int S;                           // slice capacity in shared memory (multiple of 32)
     int hi;                          // largest active set the loop takes
-    int cap;                         // rows of 6 partial sums per CTA: partial[c][cap][6]
+    int cap;                         // positions the partial-sum scratch holds: partial[cap][G][6]
     int small_hi;                    // n_act <= small_hi: lanes over sources; above: lanes over sinks
     int state;                       // != 0: the own state is resident in shared memory
     double eps2, eta, dt_min, dt_max;
@@ -274,10 +274,13 @@ __device__ __forceinline__ void gd_lp_item(const gd_dev &d, const gd_lsm &sm, in
     }
 }
 
-// element e = b * 6 + comp of the block starting at position pos -> partial[me][pos + b][comp]
-__device__ __forceinline__ void gd_lp_put(double *out, int cap, int pos, int e, double val)
+// Partial sums: partial[position][CTA][6], so that the G rows of one active particle are contiguous for its owner.
+// `out` points at this CTA's row of position 0, rs = 6 G doubles is the distance between positions.
+// element e = b * 6 + comp of the block starting at position pos -> row of position pos + b
+__device__ __forceinline__ void gd_lp_put(double *out, int rs, int pos, int e, double val)
 {
-    out[(size_t)pos * 6 + e] = val;
+    const int b = e / 6;
+    out[(size_t)(pos + b) * rs + (e - 6 * b)] = val;
 }
 
 // One work item = a register block of sinks: items 0 .. n4 - 1 hold 4 sinks, the n_act % 4 last ones hold 1.
@@ -285,7 +288,7 @@ __device__ __forceinline__ void gd_lp_put(double *out, int cap, int pos, int e, 
 // items <  warps: the rounds of every item are split over nsplit = 8 / items warps; the warp sums meet in shared
 //                 memory and are added in chunk order.
 template <bool EPS0>
-__device__ __forceinline__ void gd_lp_force_small(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int n_act, int rounds)
+__device__ __forceinline__ void gd_lp_force_small(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int rs, int n_act, int rounds)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n4 = n_act >> 2, items = n4 + (n_act & 3);
@@ -296,14 +299,14 @@ __device__ __forceinline__ void gd_lp_force_small(const gd_dev &d, const gd_lsm 
                 gd_lp_item<4, EPS0>(d, sm, 4 * it, 0, rounds, lane, la.eps2, v);
                 gd_rs24(v, lane);
                 const int e = gd_rs24_elem(lane);
-                if (e >= 0) gd_lp_put(out, la.cap, 4 * it, e, v[0]);
+                if (e >= 0) gd_lp_put(out, rs, 4 * it, e, v[0]);
             } else {
                 double v[6];
                 const int pos = 4 * n4 + (it - n4);
                 gd_lp_item<1, EPS0>(d, sm, pos, 0, rounds, lane, la.eps2, v);
                 gd_rs6(v, lane);
                 const int e = gd_rs6_elem(lane);
-                if (e >= 0) gd_lp_put(out, la.cap, pos, e, v[0]);
+                if (e >= 0) gd_lp_put(out, rs, pos, e, v[0]);
             }
         }
         return;
@@ -333,7 +336,7 @@ __device__ __forceinline__ void gd_lp_force_small(const gd_dev &d, const gd_lsm 
     if (work && chunk == 0 && lane < (four ? 24 : 6)) {
         double s = sm.red[warp * 32 + lane];
         for (int c = 1; c < nsplit; ++c) s += sm.red[(warp + c) * 32 + lane];
-        gd_lp_put(out, la.cap, pos, lane, s);
+        gd_lp_put(out, rs, pos, lane, s);
     }
 }
 
@@ -393,7 +396,7 @@ __device__ __forceinline__ int gd_lp_row_of(const gd_lsm &sm, int pos, int n, in
 }
 
 template <int BI, bool EPS0>
-__device__ __forceinline__ void gd_lp_force_wide(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int G, int n_act, int cnt_own)
+__device__ __forceinline__ void gd_lp_force_wide(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int rs, int G, int n_act, int cnt_own)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tiles = (n_act + 32 * BI - 1) / (32 * BI);
@@ -408,7 +411,7 @@ __device__ __forceinline__ void gd_lp_force_wide(const gd_dev &d, const gd_lsm &
         for (int b = 0; b < BI; ++b) {
             const int pos = tile * 32 * BI + 32 * b + lane;
             if (pos < n_act) {
-                double2 *o = reinterpret_cast<double2 *>(out + (size_t)pos * 6);
+                double2 *o = reinterpret_cast<double2 *>(out + (size_t)pos * rs);
                 o[0] = make_double2(acc[b].ax, acc[b].ay); o[1] = make_double2(acc[b].az, acc[b].jx); o[2] = make_double2(acc[b].jy, acc[b].jz);
             }
         }
@@ -416,12 +419,12 @@ __device__ __forceinline__ void gd_lp_force_wide(const gd_dev &d, const gd_lsm &
 }
 
 template <bool EPS0>
-__device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int G, int n_act, int cnt_own)
+__device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int rs, int G, int n_act, int cnt_own)
 {
     // enough sinks for every warp to hold several per lane: more independent pair chains per warp (the FP64 pipe
     // needs ~8 per scheduler to stay busy), fewer shared-memory reads per pair
-    if (n_act >= 3 * 128 * GD_LP_WARPS) { gd_lp_force_wide<4, EPS0>(d, sm, la, out, G, n_act, cnt_own); return; }
-    if (n_act >= 2 * 64 * GD_LP_WARPS) { gd_lp_force_wide<2, EPS0>(d, sm, la, out, G, n_act, cnt_own); return; }
+    if (n_act >= 3 * 128 * GD_LP_WARPS) { gd_lp_force_wide<4, EPS0>(d, sm, la, out, rs, G, n_act, cnt_own); return; }
+    if (n_act >= 2 * 64 * GD_LP_WARPS) { gd_lp_force_wide<2, EPS0>(d, sm, la, out, rs, G, n_act, cnt_own); return; }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tiles = (n_act + 31) >> 5;
     if (tiles >= GD_LP_WARPS) {
@@ -430,7 +433,7 @@ __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &s
             const gd_src si = gd_lp_load_sink(d, gd_lp_row_of(sm, min(pos, n_act - 1), la.n, G));
             const gd_acc a = gd_lp_tile<EPS0>(sm, si, 0, cnt_own, la.eps2);
             if (pos < n_act) {
-                double2 *o = reinterpret_cast<double2 *>(out + (size_t)pos * 6);
+                double2 *o = reinterpret_cast<double2 *>(out + (size_t)pos * rs);
                 o[0] = make_double2(a.ax, a.ay); o[1] = make_double2(a.az, a.jx); o[2] = make_double2(a.jy, a.jz);
             }
         }
@@ -453,7 +456,7 @@ __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &s
         for (int comp = 0; comp < 6; ++comp) {
             double s = sm.red[warp * 192 + comp * 32 + lane];
             for (int c = 1; c < nsplit; ++c) s += sm.red[(warp + c) * 192 + comp * 32 + lane];
-            out[(size_t)pos * 6 + comp] = s;
+            out[(size_t)pos * rs + comp] = s;
         }
     }
 }
@@ -485,11 +488,25 @@ __device__ __forceinline__ void gd_lp_correct_warp(const gd_dev &d, const gd_lsm
     const int i = p0 + p;
     const double4 ad = GD_LP_AD(p, i), jk = GD_LP_JK(p, i);
     double s[6] = {0, 0, 0, 0, 0, 0};
-    for (int c = lane; c < G; c += 32) {
-        const double2 *row = reinterpret_cast<const double2 *>(d.partial + ((size_t)c * la.cap + pos) * 6);
-        const double2 u0 = __ldcg(row), u1 = __ldcg(row + 1), u2 = __ldcg(row + 2);
-        s[0] += u0.x; s[1] += u0.y; s[2] += u1.x; s[3] += u1.y; s[4] += u2.x; s[5] += u2.y;
+    {   // the G rows of this position are contiguous; lane l takes rows l, l + 32, ... (48 bytes each).  Every load in
+        // flight at once (branch-free: rows beyond G are re-reads of the lane's first row with weight 0), then added in
+        // ascending c
+        const double2 *base = reinterpret_cast<const double2 *>(d.partial + (size_t)pos * 6 * G);
+        double2 v[GD_LP_MAX_GRID / 32][3];
+#pragma unroll
+        for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
+            const int c = lane + 32 * u;
+            const double2 *row = base + 3 * (c < G ? c : lane);
+            v[u][0] = __ldcg(row); v[u][1] = __ldcg(row + 1); v[u][2] = __ldcg(row + 2);
+        }
+#pragma unroll
+        for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
+            const double wgt = (lane + 32 * u < G) ? 1.0 : 0.0;
+            s[0] += wgt * v[u][0].x; s[1] += wgt * v[u][0].y; s[2] += wgt * v[u][1].x;
+            s[3] += wgt * v[u][1].y; s[4] += wgt * v[u][2].x; s[5] += wgt * v[u][2].y;
+        }
     }
+    const long long c0b = clock64() + (long long)(s[0] == 1e300);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
@@ -524,7 +541,7 @@ __device__ __forceinline__ void gd_lp_correct_warp(const gd_dev &d, const gd_lsm
             const long long c3 = clock64();
             d.lp_ctl[13] += (unsigned long long)(c1 - c0);
             d.lp_ctl[14] += (unsigned long long)(c2 - c1);
-            d.lp_ctl[15] += (unsigned long long)(c3 - c2);
+            d.lp_ctl[15] += (unsigned long long)(c0b - c0);
         }
     }
 }
@@ -536,8 +553,7 @@ __device__ __forceinline__ void gd_lp_correct_thread(const gd_dev &d, const gd_l
     const int i = p0 + p;
     const double4 ad = GD_LP_AD(p, i), jk = GD_LP_JK(p, i);
     double s[6] = {0, 0, 0, 0, 0, 0};
-    const double2 *row = reinterpret_cast<const double2 *>(d.partial + (size_t)pos * 6);
-    const size_t cs = (size_t)3 * la.cap;                    // double2 per CTA
+    const double2 *row = reinterpret_cast<const double2 *>(d.partial + (size_t)pos * 6 * G);
     // batches of 16 CTAs: 48 loads in flight, then added in ascending c
     for (int c0 = 0; c0 < G; c0 += 16) {
         double2 v[16][3];
@@ -545,7 +561,7 @@ __device__ __forceinline__ void gd_lp_correct_thread(const gd_dev &d, const gd_l
         for (int u = 0; u < 16; ++u) {
             const int c = min(c0 + u, G - 1);
 #pragma unroll
-            for (int k = 0; k < 3; ++k) v[u][k] = __ldcg(row + (size_t)c * cs + k);
+            for (int k = 0; k < 3; ++k) v[u][k] = __ldcg(row + 3 * c + k);
         }
 #pragma unroll
         for (int u = 0; u < 16; ++u) {
@@ -585,7 +601,8 @@ k_block_loop(gd_dev d, gd_largs la)
     const long long ct_steps0 = steps;
     unsigned long long *bar = d.lp_ctl;
     unsigned long long target = d.lp_ctl[1];
-    double *out = d.partial + (size_t)me * 6 * la.cap;
+    double *out = d.partial + (size_t)me * 6;
+    const int rs = 6 * G;
 
     for (int p = tid; p < rounds * 32; p += GD_LP_THREADS) {
         if (p < cnt_own) {
@@ -649,8 +666,8 @@ k_block_loop(gd_dev d, gd_largs la)
             sm.vz[p] = q.vz;
         }
         __syncthreads();
-        if (small) gd_lp_force_small<EPS0>(d, sm, la, out, n_act, rounds);
-        else gd_lp_force_big<EPS0>(d, sm, la, out, G, n_act, cnt_own);
+        if (small) gd_lp_force_small<EPS0>(d, sm, la, out, rs, n_act, rounds);
+        else gd_lp_force_big<EPS0>(d, sm, la, out, rs, G, n_act, cnt_own);
         g1 = gd_gtime(); tr[0] += g1 - g0; g0 = g1;
         gd_bar_arrive(bar);
         target += G;
