@@ -188,6 +188,19 @@ def cpu_baseline(w, t_end):
                       f"({o.particle_steps} particle steps, to t={o.t:.6g}); plain FP64 sums; {sec:.1f} s"}, sec
 
 
+def aggregate_replicas(torch, dist, device, sec, sec_e2e, pairs, pairs_e2e):
+    """Replicas only: the path does not shard, so N ranks run N independent copies of the
+    workload with no data-path collective.  The job's time is the MAX over ranks, its work the SUM over ranks.
+    dist = None: single process."""
+    if dist is None:
+        return sec, sec_e2e, pairs, pairs_e2e
+    tmax = torch.tensor([sec, sec_e2e], dtype=torch.float64, device=device)
+    dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    work = torch.tensor([pairs, pairs_e2e], dtype=torch.float64, device=device)
+    dist.all_reduce(work, op=dist.ReduceOp.SUM)
+    return tmax[0].item(), tmax[1].item(), work[0].item(), work[1].item()
+
+
 def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
 
@@ -249,12 +262,9 @@ def main_ours(args):
     barrier()
     sec_e2e = time.perf_counter() - t0
 
-    if world > 1:
-        tt = torch.tensor([sec, sec_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        sec, sec_e2e = tt.tolist()
-    pairs = sum(r["interactions"] for r in results) * world          # replicas: identical work on every rank
-    pairs_e2e = sum(r["interactions"] for r in e2e_results) * world
+    sec, sec_e2e, pairs, pairs_e2e = aggregate_replicas(
+        torch, dist if world > 1 else None, "cuda", sec, sec_e2e,
+        sum(r["interactions"] for r in results), sum(r["interactions"] for r in e2e_results))
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
