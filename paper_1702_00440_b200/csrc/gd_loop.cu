@@ -141,6 +141,7 @@ struct gd_lsm {
     double *ts;                      // [S] t_i + dt_i of the own slice
     int *lact;                       // [S] local indices of the own candidates, ascending
     int *smap;                       // [GD_LP_MAX_SMALL] active list position -> row of `rec` (small mode)
+    double2 *sink;                   // [GD_LP_MAX_SMALL][4] the sink records of the step (small mode)
     int *spre;                       // [GD_LP_MAX_GRID + 1] exclusive prefix of the contributing candidate counts
     double *red;                     // [GD_LP_WARPS][6][32] warp partial sums of a split evaluation
     double *wmin;                    // [GD_LP_WARPS]
@@ -151,7 +152,7 @@ struct gd_lsm {
 
 __host__ __device__ inline size_t gd_lsm_bytes(int S, int state)
 {
-    return (size_t)S * (16 * 3 + 8 + 8 + 4 + (state ? 128 : 0)) + GD_LP_WARPS * 6 * 32 * 8 + GD_LP_WARPS * 8 + GD_LP_MAX_SMALL * 4 +
+    return (size_t)S * (16 * 3 + 8 + 8 + 4 + (state ? 128 : 0)) + GD_LP_WARPS * 6 * 32 * 8 + GD_LP_WARPS * 8 + GD_LP_MAX_SMALL * (4 + 64) +
            (GD_LP_MAX_GRID + 1) * 4 + (GD_LP_WARPS + 1) * 4 + 66 * 4 + 64;
 }
 
@@ -173,6 +174,7 @@ __device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S, int s
     s.ts = (double *)p; p += (size_t)S * 8;
     s.red = (double *)p; p += GD_LP_WARPS * 6 * 32 * 8;
     s.wmin = (double *)p; p += GD_LP_WARPS * 8;
+    s.sink = (double2 *)p; p += GD_LP_MAX_SMALL * 64;
     s.lact = (int *)p; p += (size_t)S * 4;
     s.smap = (int *)p; p += GD_LP_MAX_SMALL * 4;
     s.spre = (int *)p; p += (GD_LP_MAX_GRID + 1) * 4;
@@ -256,7 +258,9 @@ __device__ __forceinline__ void gd_lp_item(const gd_dev &d, const gd_lsm &sm, in
     gd_acc acc[BI];
 #pragma unroll
     for (int b = 0; b < BI; ++b) {
-        si[b] = gd_lp_load_sink(d, sm.smap[pos0 + b]);
+        const double2 *row = sm.sink + 4 * (pos0 + b);
+        const double2 xy = row[0], zi = row[1], wxy = row[2], wz = row[3];
+        si[b] = gd_src{xy.x, xy.y, zi.x, 0.0, wxy.x, wxy.y, wz.x};
         acc[b] = gd_acc{0, 0, 0, 0, 0, 0};
     }
 #pragma unroll 2
@@ -655,6 +659,17 @@ k_block_loop(gd_dev d, gd_largs la)
             const int r0 = gd_slice_begin(tid, la.n, G);
             for (int k = 0; k < mine; ++k) sm.smap[excl + k] = r0 + k;
         }
+        // small mode: the sink records are fetched (L2) while the own slice is predicted
+        constexpr int NPF = GD_LP_MAX_SMALL * 4 / GD_LP_THREADS;
+        double2 pf[NPF];
+        if (small) {
+            __syncthreads();                                 // smap is complete
+#pragma unroll
+            for (int u = 0; u < NPF; ++u) {
+                const int e = tid + GD_LP_THREADS * u;
+                if (e < 4 * n_act) pf[u] = __ldcg(reinterpret_cast<const double2 *>(d.lp_rec) + 4 * (size_t)sm.smap[e >> 2] + (e & 3));
+            }
+        }
         // own slice predicted to t+
         for (int p = tid; p < cnt_own; p += GD_LP_THREADS) {
             const int i = p0 + p;
@@ -664,6 +679,13 @@ k_block_loop(gd_dev d, gd_largs la)
             sm.pzm[p] = make_double2(q.z, xm.w);
             sm.vxy[p] = make_double2(q.vx, q.vy);
             sm.vz[p] = q.vz;
+        }
+        if (small) {
+#pragma unroll
+            for (int u = 0; u < NPF; ++u) {
+                const int e = tid + GD_LP_THREADS * u;
+                if (e < 4 * n_act) sm.sink[e] = pf[u];
+            }
         }
         __syncthreads();
         if (small) gd_lp_force_small<EPS0>(d, sm, la, out, rs, n_act, rounds);
