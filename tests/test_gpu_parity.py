@@ -354,6 +354,8 @@ def test_loop_first_100_block_steps_bit_exact_schedule(gd, cfg, n):
     assert relnorm(s["a"], o.a).max() < 1e-12 and relnorm(s["j"], o.j).max() < 1e-12
     hist, diag = h.level_histogram()
     assert np.array_equal(hist, o.level_hist) and diag[0] == o.nan_count and diag[1] == o.dtmin_clamps
+    lp = h.loop_profile()
+    assert lp["block_steps"] == 100 and lp["particle_steps"] == psteps, "the persistent loop did not take the steps"
     h.close()
 
 
@@ -388,3 +390,49 @@ def test_loop_is_run_to_run_identical(gd):
         h.close()
     for k in out[0]:
         assert np.array_equal(out[0][k], out[1][k]), k
+
+
+def test_loop_tiny_systems_and_eps0(gd):
+    # N = 1, 2, 3: most CTAs own nothing; eps = 0 exercises the masked self pair inside the loop
+    z = np.zeros((1, 3))
+    h = gd.Hermite(np.array([1.0]), z, np.array([[1.0, 0, 0]]), 1e-4, 0.01)
+    h.run_until(0.5)
+    assert h.block_steps == 4 and h.loop_profile()["block_steps"] == 4
+    h.close()
+    w = W.two_body(0.5, 0.5, 1.0, 0.5)
+    h = gd.Hermite(w.m, w.x, w.v, 0.0, 0.01)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, 0.0, 0.01)
+    steps, psteps = h.run_until(2.0)
+    o.run(2.0)
+    assert steps == o.block_steps and psteps == o.particle_steps and h.loop_profile()["block_steps"] == steps
+    s = h.state_host(("x", "v", "t", "dt"))
+    assert np.array_equal(s["t"], o.t_i) and np.array_equal(s["dt"], o.dt)
+    assert np.abs(s["x"] - o.x).max() < 1e-13 and np.abs(s["v"] - o.v).max() < 1e-13
+    h.close()
+    rng = np.random.default_rng(7)
+    m, x, v = np.array([0.5, 0.3, 0.2]), rng.normal(size=(3, 3)), 0.3 * rng.normal(size=(3, 3))
+    h = gd.Hermite(m, x, v, 1e-4, 0.01)
+    o = oracle.HermiteOracle(m, x, v, 1e-4, 0.01)
+    steps, _ = h.run_until(0.25)
+    o.run(0.25)
+    s = h.state_host(("x", "t", "dt"))
+    assert steps == o.block_steps and np.array_equal(s["dt"], o.dt) and np.abs(s["x"] - o.x).max() < 1e-13
+    h.close()
+
+
+def test_loop_resumes_and_honours_max_steps(gd):
+    w = W.config(1, n=700)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    ref = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    ref.set_option("loop_max_nact", 0)
+    total = 0
+    for n in (17, 40, 33):                       # three launches of the loop, each bounded by max_steps
+        h.step(n); ref.step(n); total += n
+        assert h.block_steps == ref.block_steps == total and h.t == ref.t
+    steps, _ = h.run_until(h.t + 2.0 ** -6, max_steps=10 ** 6)
+    steps_r, _ = ref.run_until(ref.t + 2.0 ** -6, max_steps=10 ** 6)
+    assert steps == steps_r and h.t == ref.t
+    a, b = h.state_host(), ref.state_host()
+    assert np.array_equal(a["t"], b["t"]) and np.array_equal(a["dt"], b["dt"]) and np.abs(a["x"] - b["x"]).max() < 1e-12
+    assert h.loop_profile()["block_steps"] == h.block_steps
+    h.close(); ref.close()
