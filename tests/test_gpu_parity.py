@@ -436,3 +436,27 @@ def test_loop_resumes_and_honours_max_steps(gd):
     assert np.array_equal(a["t"], b["t"]) and np.array_equal(a["dt"], b["dt"]) and np.abs(a["x"] - b["x"]).max() < 1e-12
     assert h.loop_profile()["block_steps"] == h.block_steps
     h.close(); ref.close()
+
+
+def test_c2_energy_error_after_one_time_unit_matches_oracle(gd):
+    # north_star: the same |dE/E| to within 10 % after one N-body time unit (C2).  The oracle's side is stored
+    # (5 minutes of host time): tests/golden/c2_t1_energy.txt, written by tests/golden/make_c2_t1_energy.py.
+    import os
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "c2_t1_energy.txt")):
+        if not line.startswith("#"):
+            k, v = line.split()
+            gold[k] = float(v)
+    w = W.config(2)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    k0, u0 = h.energy()
+    steps, psteps = h.run_until(1.0)
+    k1, u1 = h.energy()
+    h.close()
+    # chaotic dynamics: the schedules need not stay identical for 30 k block steps (they do as of round 1)
+    assert abs(steps - gold["block_steps"]) <= 1e-3 * gold["block_steps"]
+    assert abs(psteps - gold["particle_steps"]) <= 1e-3 * gold["particle_steps"]
+    err = abs((k1 + u1) / (k0 + u0) - 1.0)
+    err_ref = abs(gold["e1"] / gold["e0"] - 1.0)
+    assert abs(k0 + u0 - gold["e0"]) <= 1e-13 * abs(gold["e0"])
+    assert abs(err - err_ref) <= 0.1 * err_ref, (err, err_ref)
