@@ -277,14 +277,14 @@ def main_ours(args):
 # (None until one exists for the workload; see profiles/README.md)
 NCU_TRAFFIC_BYTES = {("C2", "jsplit"): 938240, ("C2", "ipar"): 934656, ("C2", "ipar_small"): 936192}   # profiles/r1c_launches_graph_path.md
 KERNEL_NAMES = {"ipar": "k_force_ipar<2,1>", "jsplit": "k_force_jsplit", "ipar_small": "k_force_ipar<1,4>",
-                "loop": "k_block_loop"}
+                "loop": "k_block_loop", "slice": "k_force_slice"}
 
 
 def finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, sec_e2e, pairs, pairs_e2e, clocks,
                 prof_pass):
     K = args.steps
     prof = {k: {f: prof_pass["prof"][k][f] for f in ("launches", "ms", "pairs")}
-            for k in ("ipar", "jsplit", "ipar_small", "loop")}
+            for k in ("ipar", "jsplit", "ipar_small", "loop", "slice")}
     dom = max(prof, key=lambda k: prof[k]["ms"])
     d = prof[dom]
     achieved = FLOP_PER_PAIR * d["pairs"] / (d["ms"] * 1e-3) / 1e12 if d["ms"] > 0 else 0.0

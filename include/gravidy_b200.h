@@ -85,6 +85,11 @@ GD_API const char *gd_last_error(const gd_ctx *ctx);
  * kernel runs with 32-sink tiles, beyond it with 256-sink tiles; default 2048),
  * "dt_level_min", "dt_level_max" (override GD_LEVEL_MIN/MAX before the first step; 0 <= min <= max <= 52),
  * "halving_mode" (1: halve until dt <= dt_req [default]; 0: a single halving per step),
+ * "slice_max_nact" (active sets up to this size go to k_force_slice, one CTA per SM over a shared-memory slice of
+ * the sources, where the system is small enough for it; default 8192, 0 = off: the kernels above take over),
+ * "loop_max_nact", "loop_small_nact", "loop_state_smem" (the persistent block-step loop behind gd_step /
+ * gd_run_until: largest active set it takes [default: all], size up to which lanes stride over sources [96],
+ * own state resident in shared memory [1]),
  * "profile" (0/1: time every force launch with CUDA events, see gd_get_profile).  GD_EINVAL on unknown keys. */
 GD_API int gd_set_option(gd_ctx *ctx, const char *key, double value);
 
@@ -142,7 +147,7 @@ GD_API int64_t gd_n(const gd_ctx *ctx);
 GD_API int64_t gd_n_active(const gd_ctx *ctx);          /* size of the current internal active list */
 GD_API int64_t gd_block_steps(const gd_ctx *ctx);       /* "Iter"   of Listing 1 */
 GD_API int64_t gd_particle_steps(const gd_ctx *ctx);    /* "Nsteps" of Listing 1 */
-GD_API int     gd_last_force_kernel(const gd_ctx *ctx); /* 0 none, 1 i-parallel (256-sink tiles), 2 j-split, 3 i-parallel (32-sink tiles) */
+GD_API int     gd_last_force_kernel(const gd_ctx *ctx); /* 0 none, 1 i-parallel (256-sink tiles), 2 j-split, 3 i-parallel (32-sink tiles), 4 source-slice kernel */
 GD_API int64_t gd_kernel_launches(const gd_ctx *ctx);   /* kernels launched on behalf of this ctx so far */
 /* Launch geometry of the last explicit force evaluation -> geom_host[4] = { kernel (as above, 0 = 256-sink tiles),
  * i-tiles, source splits (i-parallel) or clusters per i-tile (j-split), units of 64 sources per split }.  Diagnostics only. */
@@ -170,8 +175,9 @@ GD_API int gd_get_loop_profile(gd_ctx *ctx, int64_t *out_host);
  * gd_force_jerk issued afterwards is bracketed by two events on the context's stream (the all-active evaluation
  * inside gd_init runs before the option can be set and is not timed); gd_step / gd_run_until then launch the
  * persistent block-step loop directly instead of replaying the graph, each launch bracketed the same way.
- * prof_host[16] receives, for kind k = 0 (i-parallel kernel, 256-sink tiles), 1 (j-split kernel), 2 (i-parallel
- * kernel, 32-sink tiles), 3 (k_block_loop: pairs = particle steps taken inside the loop x n):
+ * prof_host[20] receives, for kind k = 0 (i-parallel kernel, 256-sink tiles), 1 (j-split kernel), 2 (i-parallel
+ * kernel, 32-sink tiles), 3 (k_block_loop: pairs = particle steps taken inside the loop x n), 4 (k_force_slice,
+ * with its fold kernel):
  *   prof[4k] launches timed, prof[4k+1] sum of durations in ms, prof[4k+2] sum of pair interactions (n_act * n),
  *   prof[4k+3] sum of squared durations (ms^2).  Synchronises on the last recorded event. */
 GD_API int gd_get_profile(gd_ctx *ctx, double *prof_host);

@@ -253,7 +253,7 @@ class Hermite:
 
     @property
     def last_force_kernel(self) -> str:
-        return {0: "none", 1: "ipar", 2: "jsplit", 3: "ipar_small"}[int(self._lib.gd_last_force_kernel(self._h))]
+        return {0: "none", 1: "ipar", 2: "jsplit", 3: "ipar_small", 4: "slice"}[int(self._lib.gd_last_force_kernel(self._h))]
 
     @property
     def kernel_launches(self) -> int:
@@ -298,10 +298,10 @@ class Hermite:
 
     def profile(self) -> dict:
         """Event-timed force launches since the "profile" option was set: per kernel launches, ms, pairs."""
-        p = np.zeros(16)
+        p = np.zeros(20)
         self._check(self._lib.gd_get_profile(self._h, p.ctypes.data))
         return {k: {"launches": int(p[4 * i]), "ms": float(p[4 * i + 1]), "pairs": float(p[4 * i + 2]),
-                    "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit", "ipar_small", "loop"))}
+                    "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit", "ipar_small", "loop", "slice"))}
 
     def loop_profile(self) -> dict:
         o = np.zeros(14, dtype=np.int64)

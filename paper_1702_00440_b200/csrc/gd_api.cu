@@ -180,6 +180,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->ipar_small_max_nact = 2048;
     c->loop_max_nact = (int64_t)1 << 40;      // every step the scratch allows
     c->loop_small_nact = 96;
+    c->slice_max_nact = 8192;
     c->loop_state_opt = 1;
     c->stream = (cudaStream_t)stream;
     gd_carve(&c->d, ws, c->np, c->pcap);
@@ -204,6 +205,7 @@ static int gd_prepare(gd_ctx *c)
     GD_CUDA(c, cudaMemsetAsync(c->d.blockmin, 0, (char *)c->d.phi - (char *)c->d.blockmin, c->stream));
     int rc = gdk_force_setup(c);
     if (!rc) rc = gdk_loop_setup(c);
+    if (!rc) rc = gdk_slice_setup(c);
     return rc;
 }
 
@@ -262,6 +264,7 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
     if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "ipar_small_max_nact")) { c->ipar_small_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "use_graph")) { c->use_graph = value != 0.0; return GD_OK; }
+    if (!strcmp(key, "slice_max_nact")) { c->slice_max_nact = (int64_t)value; return GD_OK; }
     if (!strcmp(key, "loop_max_nact") || !strcmp(key, "loop_small_nact") || !strcmp(key, "loop_state_smem")) {
         if (!strcmp(key, "loop_max_nact")) c->loop_max_nact = (int64_t)value;
         else if (!strcmp(key, "loop_small_nact")) c->loop_small_nact = (int64_t)value;

@@ -87,6 +87,9 @@ struct gd_ctx {
     int64_t loop_small_nact;             // option: active sets up to this size use the lanes-over-sources mapping
     int loop_grid, loop_S, loop_hi, loop_cap, loop_state;   // geometry of k_block_loop (loop_grid = 0: not usable)
     size_t loop_smem;
+    int64_t slice_max_nact;              // option: largest active set gd_force_jerk gives to k_force_slice (0 = off)
+    int slice_grid, slice_S;             // geometry of k_force_slice (slice_grid = 0: not usable)
+    size_t slice_smem;
     int64_t graph_nodes;                 // kernel nodes in step_graph
     int sm_count;
     // optional CUDA-event timing of the force launches ("profile" option; see gd_get_profile)
@@ -96,7 +99,7 @@ struct gd_ctx {
     int ev_kind[GD_PROF_POOL];
     int ev_pending;
     bool ev_created;
-    double prof[16];             // per kind k = 0 (i-parallel L), 1 (j-split), 2 (i-parallel S), 3 (block-step loop): {launches, ms, pairs, ms^2}
+    double prof[20];             // per kind k = 0 (i-parallel L), 1 (j-split), 2 (i-parallel S), 3 (block-step loop), 4 (slice): {launches, ms, pairs, ms^2}
     char err[512];
 };
 
@@ -121,6 +124,9 @@ int gdk_correct(gd_ctx *c, double t_next, bool dev = false);                    
 int gdk_next_block(gd_ctx *c, bool dev = false);                                             // gd_next_block.cu
 int gdk_loop_setup(gd_ctx *c);                                                               // gd_loop.cu
 int gdk_loop(gd_ctx *c);
+int gdk_slice_setup(gd_ctx *c);
+int64_t gdk_slice_hi(const gd_ctx *c);
+int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out);
 int gdk_energy(gd_ctx *c);                                                                   // gd_energy.cu
 int gdk_fp64_probe(int iters, double *flops, double *ms);                                    // gd_probe.cu
 

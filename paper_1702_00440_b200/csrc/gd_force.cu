@@ -582,10 +582,13 @@ int gdk_force(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, doubl
 {
     if (n_act <= 0) return 0;
     const int js_hi = gd_js_hi(c), s_hi = gd_s_hi(c);
-    const int kind = n_act <= js_hi ? 1 : (n_act <= s_hi ? 2 : 0);
+    const int kind = n_act <= gdk_slice_hi(c) ? 4 : (n_act <= js_hi ? 1 : (n_act <= s_hi ? 2 : 0));
     const int slot = gd_prof_begin(c);
     int rc;
-    if (kind == 1) {
+    if (kind == 4) {
+        rc = gdk_force_slice(c, idx, n_act, a_out, j_out);
+        c->last_geom[0] = 4; c->last_geom[1] = c->slice_grid; c->last_geom[2] = c->slice_S; c->last_geom[3] = 0;
+    } else if (kind == 1) {
         int64_t i_tiles = (n_act + 31) / 32;
         rc = gd_launch_jsplit(c, gd_make_fargs(c, idx, n_act, false, 0, INT_MAX, nullptr, a_out, j_out), c->js_clusters);
         c->last_geom[0] = 1; c->last_geom[1] = (int)i_tiles; c->last_geom[2] = c->js_clusters / (int)i_tiles; c->last_geom[3] = 0;
@@ -600,7 +603,7 @@ int gdk_force(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, doubl
         rc = gd_launch_ipar<2, 1>(c, gd_make_fargs(c, idx, n_act, false, 0, INT_MAX, c->d.geom_l, a_out, j_out), grid);
         c->last_geom[0] = 0; c->last_geom[1] = (int)i_tiles; c->last_geom[2] = c->h_geom_l[2 * i_tiles]; c->last_geom[3] = c->h_geom_l[2 * i_tiles + 1];
     }
-    c->last_force_kernel = kind == 1 ? 2 : (kind == 2 ? 3 : 1);
+    c->last_force_kernel = kind == 4 ? 4 : (kind == 1 ? 2 : (kind == 2 ? 3 : 1));
     gd_prof_end(c, slot, kind, (double)n_act * (double)c->n);
     return rc;
 }

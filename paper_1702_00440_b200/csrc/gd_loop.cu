@@ -43,6 +43,8 @@ struct gd_largs {
     int state;                       // != 0: the own state is resident in shared memory
     double eps2, eta, dt_min, dt_max;
     int halving_mode;
+    int ext;                         // != 0 (k_force_slice): the sinks are named by ext_idx in the predicted planes
+    const int32_t *ext_idx;          //   (NULL: sink k = particle k); 0 (k_block_loop): they are the published records
 };
 
 __device__ __forceinline__ int gd_slice_begin(int c, int n, int G) { return (int)((long long)c * n / G); }
@@ -143,7 +145,7 @@ struct gd_lsm {
     int *smap;                       // [GD_LP_MAX_SMALL] active list position -> row of `rec` (small mode)
     double2 *sink;                   // [GD_LP_MAX_SMALL][4] the sink records of the step (small mode)
     int *spre;                       // [GD_LP_MAX_GRID + 1] exclusive prefix of the contributing candidate counts
-    double *red;                     // [GD_LP_WARPS][6][32] warp partial sums of a split evaluation
+    double *red;                     // [GD_LP_WARPS][4][6][32] warp partial sums of a split evaluation
     double *wmin;                    // [GD_LP_WARPS]
     int *wcnt;                       // [GD_LP_WARPS + 1]
     unsigned int *hist;              // [64] particle steps per level, [64..65] diagnostics
@@ -152,7 +154,7 @@ struct gd_lsm {
 
 __host__ __device__ inline size_t gd_lsm_bytes(int S, int state)
 {
-    return (size_t)S * (16 * 3 + 8 + 8 + 4 + (state ? 128 : 0)) + GD_LP_WARPS * 6 * 32 * 8 + GD_LP_WARPS * 8 + GD_LP_MAX_SMALL * (4 + 64) +
+    return (size_t)S * (16 * 3 + 8 + 8 + 4 + (state ? 128 : 0)) + GD_LP_WARPS * 4 * 6 * 32 * 8 + GD_LP_WARPS * 8 + GD_LP_MAX_SMALL * (4 + 64) +
            (GD_LP_MAX_GRID + 1) * 4 + (GD_LP_WARPS + 1) * 4 + 66 * 4 + 64;
 }
 
@@ -172,7 +174,7 @@ __device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S, int s
     s.vxy = (double2 *)p; p += (size_t)S * 16;
     s.vz = (double *)p; p += (size_t)S * 8;
     s.ts = (double *)p; p += (size_t)S * 8;
-    s.red = (double *)p; p += GD_LP_WARPS * 6 * 32 * 8;
+    s.red = (double *)p; p += GD_LP_WARPS * 4 * 6 * 32 * 8;
     s.wmin = (double *)p; p += GD_LP_WARPS * 8;
     s.sink = (double2 *)p; p += GD_LP_MAX_SMALL * 64;
     s.lact = (int *)p; p += (size_t)S * 4;
@@ -345,9 +347,7 @@ __device__ __forceinline__ void gd_lp_force_small(const gd_dev &d, const gd_lsm 
 }
 
 // ---- [force], big mode: lanes hold sinks, the own sources are read by broadcast --------------------------------------
-// Tile = 32 consecutive active-list positions.  tiles >= warps: warp w takes tiles w, w + 8, ... against the whole
-// slice; fewer tiles: the slice is split over nsplit = 8 / tiles warps per tile and the warp sums are added in chunk
-// order in shared memory.  Two independent accumulator sets (even / odd sources) keep the FP64 pipe fed.
+// narrow tiles: one sink per lane, two independent accumulator sets (even / odd sources)
 template <bool EPS0>
 __device__ __forceinline__ gd_acc gd_lp_tile(const gd_lsm &sm, const gd_src &si, int jb, int je, double eps2)
 {
@@ -372,14 +372,14 @@ __device__ __forceinline__ gd_acc gd_lp_tile(const gd_lsm &sm, const gd_src &si,
     return a0;
 }
 
-// wide tiles: BI sinks per lane (positions pos0 + 32 b + lane) against the whole slice, one accumulator set per sink
+// wide tiles: BI sinks per lane (positions pos0 + 32 b + lane) against the sources [jb, je), one accumulator set per sink
 template <int BI, bool EPS0>
-__device__ __forceinline__ void gd_lp_tile_wide(const gd_lsm &sm, const gd_src (&si)[BI], int cnt, double eps2, gd_acc (&acc)[BI])
+__device__ __forceinline__ void gd_lp_tile_wide(const gd_lsm &sm, const gd_src (&si)[BI], int jb, int je, double eps2, gd_acc (&acc)[BI])
 {
 #pragma unroll
     for (int b = 0; b < BI; ++b) acc[b] = gd_acc{0, 0, 0, 0, 0, 0};
 #pragma unroll 2
-    for (int j = 0; j < cnt; ++j) {
+    for (int j = jb; j < je; ++j) {
         const double2 xy = sm.pxy[j], zm = sm.pzm[j], vxy = sm.vxy[j];
         const gd_src sj{xy.x, xy.y, zm.x, zm.y, vxy.x, vxy.y, sm.vz[j]};
 #pragma unroll
@@ -399,42 +399,105 @@ __device__ __forceinline__ int gd_lp_row_of(const gd_lsm &sm, int pos, int n, in
     return gd_slice_begin(lo, n, G) + (pos - sm.spre[lo]);
 }
 
+// sink at a position of the active list
+__device__ __forceinline__ gd_src gd_lp_sink_at(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, int pos, int G)
+{
+    if (la.ext) {
+        const int i = la.ext_idx ? __ldg(la.ext_idx + pos) : pos;
+        const double2 xy = __ldg(d.pxy + i), zm = __ldg(d.pzm + i), vxy = __ldg(d.vxy + i);
+        return gd_src{xy.x, xy.y, zm.x, 0.0, vxy.x, vxy.y, __ldg(d.vz + i)};
+    }
+    return gd_lp_load_sink(d, gd_lp_row_of(sm, pos, la.n, G));
+}
+
+// Tiles of 32 BI consecutive positions, BI sinks per lane: BI independent pair chains per warp (the FP64 pipe needs
+// ~8 per scheduler to stay busy) and one shared-memory read of a source per BI pairs.  tiles >= warps: warp w takes
+// tiles w, w + 8, ... against the whole slice.  Fewer tiles: see below.
 template <int BI, bool EPS0>
 __device__ __forceinline__ void gd_lp_force_wide(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int rs, int G, int n_act, int cnt_own)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tiles = (n_act + 32 * BI - 1) / (32 * BI);
-    for (int tile = warp; tile < tiles; tile += GD_LP_WARPS) {
+    if (tiles >= GD_LP_WARPS) {
+        for (int tile = warp; tile < tiles; tile += GD_LP_WARPS) {
+            gd_src si[BI];
+            gd_acc acc[BI];
+#pragma unroll
+            for (int b = 0; b < BI; ++b) si[b] = gd_lp_sink_at(d, sm, la, min(tile * 32 * BI + 32 * b + lane, n_act - 1), G);
+            gd_lp_tile_wide<BI, EPS0>(sm, si, 0, cnt_own, la.eps2, acc);
+#pragma unroll
+            for (int b = 0; b < BI; ++b) {
+                const int pos = tile * 32 * BI + 32 * b + lane;
+                if (pos < n_act) {
+                    double2 *o = reinterpret_cast<double2 *>(out + (size_t)pos * rs);
+                    o[0] = make_double2(acc[b].ax, acc[b].ay); o[1] = make_double2(acc[b].az, acc[b].jx); o[2] = make_double2(acc[b].jy, acc[b].jz);
+                }
+            }
+        }
+        return;
+    }
+    // fewer tiles than warps: the slice is split over nsplit = 8 / tiles warps per tile; the warp sums meet in shared
+    // memory and are added in chunk order
+    const int nsplit = GD_LP_WARPS / tiles;
+    const int tile = warp / nsplit, chunk = warp - tile * nsplit;
+    const bool work = tile < tiles;
+    if (work) {
         gd_src si[BI];
         gd_acc acc[BI];
 #pragma unroll
-        for (int b = 0; b < BI; ++b)
-            si[b] = gd_lp_load_sink(d, gd_lp_row_of(sm, min(tile * 32 * BI + 32 * b + lane, n_act - 1), la.n, G));
-        gd_lp_tile_wide<BI, EPS0>(sm, si, cnt_own, la.eps2, acc);
+        for (int b = 0; b < BI; ++b) si[b] = gd_lp_sink_at(d, sm, la, min(tile * 32 * BI + 32 * b + lane, n_act - 1), G);
+        const int jb = (int)((long long)cnt_own * chunk / nsplit), je = (int)((long long)cnt_own * (chunk + 1) / nsplit);
+        gd_lp_tile_wide<BI, EPS0>(sm, si, jb, je, la.eps2, acc);
+#pragma unroll
+        for (int b = 0; b < BI; ++b) {
+            double *r = sm.red + (warp * 4 + b) * 192 + lane;
+            r[0] = acc[b].ax; r[32] = acc[b].ay; r[64] = acc[b].az; r[96] = acc[b].jx; r[128] = acc[b].jy; r[160] = acc[b].jz;
+        }
+    }
+    __syncthreads();
+    if (work && chunk == 0) {
 #pragma unroll
         for (int b = 0; b < BI; ++b) {
             const int pos = tile * 32 * BI + 32 * b + lane;
             if (pos < n_act) {
-                double2 *o = reinterpret_cast<double2 *>(out + (size_t)pos * rs);
-                o[0] = make_double2(acc[b].ax, acc[b].ay); o[1] = make_double2(acc[b].az, acc[b].jx); o[2] = make_double2(acc[b].jy, acc[b].jz);
+#pragma unroll
+                for (int comp = 0; comp < 6; ++comp) {
+                    double sum = sm.red[(warp * 4 + b) * 192 + comp * 32 + lane];
+                    for (int c = 1; c < nsplit; ++c) sum += sm.red[((warp + c) * 4 + b) * 192 + comp * 32 + lane];
+                    out[(size_t)pos * rs + comp] = sum;
+                }
             }
         }
     }
 }
 
+// share of the warps that work when `tiles` tiles are dealt to 8 warps (tiles < 8: the sources are split instead)
+__device__ __forceinline__ int gd_lp_balance(int tiles)
+{
+    if (tiles < GD_LP_WARPS) return 100 * (tiles * (GD_LP_WARPS / tiles)) / GD_LP_WARPS;
+    return 100 * tiles / (GD_LP_WARPS * ((tiles + GD_LP_WARPS - 1) / GD_LP_WARPS));
+}
+
 template <bool EPS0>
 __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int rs, int G, int n_act, int cnt_own)
 {
-    // enough sinks for every warp to hold several per lane: more independent pair chains per warp (the FP64 pipe
-    // needs ~8 per scheduler to stay busy), fewer shared-memory reads per pair
-    if (n_act >= 3 * 128 * GD_LP_WARPS) { gd_lp_force_wide<4, EPS0>(d, sm, la, out, rs, G, n_act, cnt_own); return; }
-    if (n_act >= 2 * 64 * GD_LP_WARPS) { gd_lp_force_wide<2, EPS0>(d, sm, la, out, rs, G, n_act, cnt_own); return; }
+    // Wide tiles (2 or 4 sinks per lane: more independent pair chains per warp, fewer shared-memory reads per pair)
+    // wherever they still deal the work evenly: always from 1024 sinks on, and below that when the slice is long
+    // enough to be split over the warps of a tile (measured: N = 65536, 256 sinks: 44 us against 76 us with narrow
+    // tiles; N = 16384 the other way round).
+    if (n_act >= 2 * 64 * GD_LP_WARPS || cnt_own >= 256) {
+        if (gd_lp_balance((n_act + 127) >> 7) + 5 >= gd_lp_balance((n_act + 63) >> 6))
+            gd_lp_force_wide<4, EPS0>(d, sm, la, out, rs, G, n_act, cnt_own);
+        else
+            gd_lp_force_wide<2, EPS0>(d, sm, la, out, rs, G, n_act, cnt_own);
+        return;
+    }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tiles = (n_act + 31) >> 5;
     if (tiles >= GD_LP_WARPS) {
         for (int tile = warp; tile < tiles; tile += GD_LP_WARPS) {
             const int pos = tile * 32 + lane;
-            const gd_src si = gd_lp_load_sink(d, gd_lp_row_of(sm, min(pos, n_act - 1), la.n, G));
+            const gd_src si = gd_lp_sink_at(d, sm, la, min(pos, n_act - 1), G);
             const gd_acc a = gd_lp_tile<EPS0>(sm, si, 0, cnt_own, la.eps2);
             if (pos < n_act) {
                 double2 *o = reinterpret_cast<double2 *>(out + (size_t)pos * rs);
@@ -448,7 +511,7 @@ __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &s
     const bool work = tile < tiles;
     const int pos = tile * 32 + lane;
     if (work) {
-        const gd_src si = gd_lp_load_sink(d, gd_lp_row_of(sm, min(pos, n_act - 1), la.n, G));
+        const gd_src si = gd_lp_sink_at(d, sm, la, min(pos, n_act - 1), G);
         const int jb = (int)((long long)cnt_own * chunk / nsplit), je = (int)((long long)cnt_own * (chunk + 1) / nsplit);
         const gd_acc a = gd_lp_tile<EPS0>(sm, si, jb, je, la.eps2);
         double *r = sm.red + warp * 192 + lane;
@@ -464,6 +527,7 @@ __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &s
         }
     }
 }
+
 
 // ---- [correct] -----------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void gd_lp_commit(const gd_dev &d, const gd_lsm &sm, int i, int p, double m, const gd_corrected &r,
@@ -740,6 +804,122 @@ k_block_loop(gd_dev d, gd_largs la)
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------------
+// k_force_slice: the loop's force phase as a stage kernel for gd_force_jerk (steps a3 / a4 with an explicit or the
+// internal active list): one CTA per SM takes a slice of the np predicted source records into shared memory and
+// evaluates the partial sums of EVERY listed sink against it, with the mappings above.  The partial rows are folded
+//   n_act <= 16:  by the last CTA to finish (ticket), a warp per sink over the G contiguous rows of its position;
+//   larger:       by k_fold_slice_warp, the same with a warp per sink over the whole machine (one coalesced read each).
+#define GD_SL_TICKET_MAX 16
+struct gd_sargs {
+    int n_act;
+    double *a_out, *j_out;           // [n_act,3]
+    unsigned int *ticket;
+};
+
+template <bool EPS0>
+__global__ void __launch_bounds__(GD_LP_THREADS, 1)
+k_force_slice(gd_dev d, gd_largs la, gd_sargs sa)
+{
+    extern __shared__ __align__(16) unsigned char gd_lp_smem[];
+    __shared__ bool s_last;
+    const gd_lsm sm = gd_lsm_carve(gd_lp_smem, la.S, 0);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int G = gridDim.x, me = blockIdx.x;
+    const int n_act = sa.n_act;
+    const int p0 = gd_slice_begin(me, la.n, G);
+    const int cnt_own = gd_slice_begin(me + 1, la.n, G) - p0;
+    const int rounds = (cnt_own + 31) / 32;
+    const bool small = n_act <= la.small_hi;
+    for (int p = tid; p < rounds * 32; p += GD_LP_THREADS) {
+        const bool in = p < cnt_own;
+        sm.pxy[p] = in ? d.pxy[p0 + p] : make_double2(0.0, 0.0);
+        sm.pzm[p] = in ? d.pzm[p0 + p] : make_double2(0.0, 0.0);
+        sm.vxy[p] = in ? d.vxy[p0 + p] : make_double2(0.0, 0.0);
+        sm.vz[p] = in ? d.vz[p0 + p] : 0.0;
+    }
+    if (small) {
+        for (int e = tid; e < 4 * n_act; e += GD_LP_THREADS) {
+            const int pos = e >> 2, part = e & 3;
+            const int i = la.ext_idx ? __ldg(la.ext_idx + pos) : pos;
+            double2 v;
+            if (part == 0) v = __ldg(d.pxy + i);
+            else if (part == 1) v = __ldg(d.pzm + i);
+            else if (part == 2) v = __ldg(d.vxy + i);
+            else v = make_double2(__ldg(d.vz + i), 0.0);
+            sm.sink[e] = v;
+        }
+    }
+    __syncthreads();
+    const size_t ps = (size_t)6 * G;
+    double *out = d.partial + (size_t)me * 6;
+    if (small) gd_lp_force_small<EPS0>(d, sm, la, out, (int)ps, n_act, rounds);
+    else gd_lp_force_big<EPS0>(d, sm, la, out, (int)ps, G, n_act, cnt_own);
+    if (n_act > GD_SL_TICKET_MAX) return;
+
+    // a handful of sinks: the last CTA to arrive folds; a warp per sink, lanes over the G contiguous rows of its position
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        const unsigned int tk = atomicAdd(sa.ticket, 1u);
+        s_last = (tk == (unsigned int)G - 1u);
+        if (s_last) *sa.ticket = 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    for (int pos = warp; pos < n_act; pos += GD_LP_WARPS) {
+        const double *base = d.partial + (size_t)pos * ps;
+        double s[6] = {0, 0, 0, 0, 0, 0};
+        for (int c = lane; c < G; c += 32) {
+            const double2 *row = reinterpret_cast<const double2 *>(base + (size_t)c * 6);
+            const double2 u0 = __ldcg(row), u1 = __ldcg(row + 1), u2 = __ldcg(row + 2);
+            s[0] += u0.x; s[1] += u0.y; s[2] += u1.x; s[3] += u1.y; s[4] += u2.x; s[5] += u2.y;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+            for (int k = 0; k < 6; ++k) s[k] += __shfl_xor_sync(GD_FULL, s[k], o);
+        }
+        if (lane == 0) {
+            sa.a_out[3 * (size_t)pos] = s[0]; sa.a_out[3 * (size_t)pos + 1] = s[1]; sa.a_out[3 * (size_t)pos + 2] = s[2];
+            sa.j_out[3 * (size_t)pos] = s[3]; sa.j_out[3 * (size_t)pos + 1] = s[4]; sa.j_out[3 * (size_t)pos + 2] = s[5];
+        }
+    }
+}
+
+// partial[pos][c][6] -> a_out, j_out; one warp per sink: lanes stride over the G contiguous rows, fixed butterfly
+__global__ void __launch_bounds__(GD_LP_THREADS)
+k_fold_slice_warp(gd_dev d, int G, gd_sargs sa)
+{
+    const int lane = threadIdx.x & 31, pos = blockIdx.x * GD_LP_WARPS + (threadIdx.x >> 5);
+    if (pos >= sa.n_act) return;
+    const double2 *base = reinterpret_cast<const double2 *>(d.partial + (size_t)pos * 6 * G);
+    double2 v[GD_LP_MAX_GRID / 32][3];
+#pragma unroll
+    for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
+        const int c = lane + 32 * u;
+        const double2 *row = base + 3 * (c < G ? c : lane);
+        v[u][0] = __ldcg(row); v[u][1] = __ldcg(row + 1); v[u][2] = __ldcg(row + 2);
+    }
+    double s[6] = {0, 0, 0, 0, 0, 0};
+#pragma unroll
+    for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
+        const double wgt = (lane + 32 * u < G) ? 1.0 : 0.0;
+        s[0] += wgt * v[u][0].x; s[1] += wgt * v[u][0].y; s[2] += wgt * v[u][1].x;
+        s[3] += wgt * v[u][1].y; s[4] += wgt * v[u][2].x; s[5] += wgt * v[u][2].y;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) s[k] += __shfl_xor_sync(GD_FULL, s[k], o);
+    }
+    if (lane == 0) {
+        sa.a_out[3 * (size_t)pos] = s[0]; sa.a_out[3 * (size_t)pos + 1] = s[1]; sa.a_out[3 * (size_t)pos + 2] = s[2];
+        sa.j_out[3 * (size_t)pos] = s[3]; sa.j_out[3 * (size_t)pos + 1] = s[4]; sa.j_out[3 * (size_t)pos + 2] = s[5];
+    }
+}
+
 // ---- host side ------------------------------------------------------------------------------------------------------------
 // Geometry: one CTA per SM; S = slice capacity (multiple of 32); hi = largest active set taken, bounded by the option
 // `loop_max_nact` and by the partial-sum scratch (grid x 6 x cap doubles).  loop_grid = 0: the loop is not usable
@@ -794,10 +974,76 @@ int gdk_loop(gd_ctx *c)
     la.dt_min = c->dt_min;
     la.dt_max = c->dt_max;
     la.halving_mode = c->halving_mode;
+    la.ext = 0;
+    la.ext_idx = nullptr;
     void *args[] = {(void *)&c->d, (void *)&la};
     const void *fn = (c->eps2 < 2.3e-308) ? (const void *)k_block_loop<true> : (const void *)k_block_loop<false>;
     cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)c->loop_grid), dim3(GD_LP_THREADS), args, c->loop_smem, c->stream);
     if (e != cudaSuccess) return gd_fail_cuda(c, e, "k_block_loop");
     c->launches += 1;
+    return 0;
+}
+
+// ---- k_force_slice: host side -------------------------------------------------------------------------------------------
+int gdk_slice_setup(gd_ctx *c)
+{
+    c->slice_grid = 0;
+    int grid = c->sm_count < GD_LP_MAX_GRID ? c->sm_count : GD_LP_MAX_GRID;
+    if (grid < 1 || c->n > INT_MAX / 2) return 0;
+    int64_t S = (c->n + grid - 1) / grid;
+    S = (S + 31) / 32 * 32;
+    int dev = 0, max_smem = 0;
+    GD_CUDA(c, cudaGetDevice(&dev));
+    GD_CUDA(c, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    const size_t bytes = gd_lsm_bytes((int)S, 0);
+    if (bytes > (size_t)max_smem) return 0;
+    GD_CUDA(c, cudaFuncSetAttribute(k_force_slice<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    GD_CUDA(c, cudaFuncSetAttribute(k_force_slice<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    c->slice_grid = grid;
+    c->slice_S = (int)S;
+    c->slice_smem = bytes;
+    return 0;
+}
+
+// largest active set k_force_slice can take: option `slice_max_nact`, one partial row per (CTA, sink)
+int64_t gdk_slice_hi(const gd_ctx *c)
+{
+    if (c->slice_grid < 1) return 0;
+    int64_t hi = c->slice_max_nact < c->np ? c->slice_max_nact : c->np;
+    const int64_t cap = c->pcap / c->slice_grid / 32 * 32;
+    return hi < cap ? hi : cap;
+}
+
+int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out)
+{
+    gd_largs la;
+    la.n = (int)c->n;
+    la.S = c->slice_S;
+    la.hi = (int)n_act;
+    la.cap = (int)((n_act + 31) / 32 * 32);
+    int64_t sh = c->loop_small_nact < GD_LP_MAX_SMALL ? c->loop_small_nact : GD_LP_MAX_SMALL;
+    la.small_hi = (int)(sh < 0 ? 0 : sh);
+    la.state = 0;
+    la.eps2 = c->eps2;
+    la.eta = c->eta;
+    la.dt_min = c->dt_min;
+    la.dt_max = c->dt_max;
+    la.halving_mode = c->halving_mode;
+    la.ext = 1;
+    la.ext_idx = idx;
+    gd_sargs sa;
+    sa.n_act = (int)n_act;
+    sa.a_out = a_out;
+    sa.j_out = j_out;
+    sa.ticket = c->d.work + 2;
+    if (c->eps2 < 2.3e-308)
+        k_force_slice<true><<<c->slice_grid, GD_LP_THREADS, c->slice_smem, c->stream>>>(c->d, la, sa);
+    else
+        k_force_slice<false><<<c->slice_grid, GD_LP_THREADS, c->slice_smem, c->stream>>>(c->d, la, sa);
+    GD_LAUNCH_CHECK(c, "k_force_slice");
+    if (n_act > GD_SL_TICKET_MAX) {
+        k_fold_slice_warp<<<(unsigned)((n_act + GD_LP_WARPS - 1) / GD_LP_WARPS), GD_LP_THREADS, 0, c->stream>>>(c->d, c->slice_grid, sa);
+        GD_LAUNCH_CHECK(c, "k_fold_slice_warp");
+    }
     return 0;
 }

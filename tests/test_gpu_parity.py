@@ -74,15 +74,16 @@ def test_force_all_active_configs(gd, cfg, n):
     assert ea.max() <= TOL and ej.max() <= TOL, (ea.max(), ej.max())
 
 
-KERNEL_OPTIONS = {   # force one of the three force kernels regardless of n_act
-    "ipar": {"jsplit_max_nact": 0, "ipar_small_max_nact": 0},
-    "ipar_small": {"jsplit_max_nact": 0, "ipar_small_max_nact": 1 << 30},
-    "jsplit": {"jsplit_max_nact": 1 << 30},      # capped by the library at 32 sinks x the clusters of its grid
+KERNEL_OPTIONS = {   # force one of the four force kernels regardless of n_act
+    "ipar": {"slice_max_nact": 0, "jsplit_max_nact": 0, "ipar_small_max_nact": 0},
+    "ipar_small": {"slice_max_nact": 0, "jsplit_max_nact": 0, "ipar_small_max_nact": 1 << 30},
+    "jsplit": {"slice_max_nact": 0, "jsplit_max_nact": 1 << 30},   # capped by the library at 32 sinks x the clusters of its grid
+    "slice": {"slice_max_nact": 1 << 30},
 }
 
 
-@pytest.mark.parametrize("kernel", ["ipar", "ipar_small", "jsplit"])
-@pytest.mark.parametrize("n_act", [1, 5, 16, 100, 256, 1000, 4096])
+@pytest.mark.parametrize("kernel", ["ipar", "ipar_small", "jsplit", "slice"])
+@pytest.mark.parametrize("n_act", [1, 5, 16, 96, 97, 100, 256, 1000, 4096])
 def test_force_active_subsets_all_kernels(gd, kernel, n_act):
     # C3-style index sets on a smaller sphere, forced through each kernel; all must agree with the oracle
     import torch
@@ -308,6 +309,7 @@ def test_graph_replay_equals_explicit_calls(gd, cfg, n):
     he = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
     hg.set_option("loop_max_nact", 0)            # stage kernels only: the persistent loop sums in another order
     he.set_option("use_graph", 0)
+    he.set_option("slice_max_nact", 0)           # ... and so does k_force_slice, which the graph does not hold
     for steps in (40, 70):                       # 70 is not a multiple of the graph's step count
         pg = hg.step(steps)
         pe = he.step(steps)
