@@ -165,7 +165,7 @@ GD_API int gd_get_active(gd_ctx *ctx, int32_t *idx_dev, int64_t cap);
  * diag_host[2] = { time-step criteria that evaluated to NaN, clamps at dt_min }.  Synchronises. */
 GD_API int gd_get_level_histogram(gd_ctx *ctx, int64_t *counts_host, int64_t *diag_host);
 /* Counters of the persistent block-step loop (k_block_loop, the kernel behind gd_step / gd_run_until that takes the
- * block steps with small active sets) since init -> out_host[8] = { particle steps, block steps taken inside
+ * block steps) since init -> out_host[11] = { particle steps, block steps taken inside
  * the loop, ns spent inside it (device global timer, CTA 0), ns in its force phase, in the barrier after it, in its
  * corrector phase, in the barrier after it, launches that did work, and for CTA 0 as an owner of active particles:
  * steps, ns summing partials + correcting, ns publishing } (11 values).  Synchronises. */

@@ -304,10 +304,10 @@ class Hermite:
                     "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit", "ipar_small", "loop", "slice"))}
 
     def loop_profile(self) -> dict:
-        o = np.zeros(14, dtype=np.int64)
+        o = np.zeros(11, dtype=np.int64)
         self._check(self._lib.gd_get_loop_profile(self._h, o.ctypes.data))
         keys = ("particle_steps", "block_steps", "ns", "ns_force", "ns_barrier1", "ns_correct", "ns_barrier2", "launches",
-                "owner_steps", "ns_owner_correct", "ns_owner_publish", "clk_sum", "clk_corr", "clk_commit")
+                "owner_steps", "ns_owner_correct", "ns_owner_publish")
         return {k: int(v) for k, v in zip(keys, o)}
 
     def level_histogram(self) -> tuple[np.ndarray, np.ndarray]:

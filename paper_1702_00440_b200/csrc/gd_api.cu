@@ -611,7 +611,7 @@ extern "C" int gd_get_profile(gd_ctx *c, double *prof_host)
 extern "C" int gd_get_loop_profile(gd_ctx *c, int64_t *out_host)
 {
     if (!c || !out_host) return GD_EINVAL;
-    GD_CUDA(c, cudaMemcpyAsync(out_host, c->d.lp_ctl + 2, 14 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaMemcpyAsync(out_host, c->d.lp_ctl + 2, 11 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
     GD_CUDA(c, cudaStreamSynchronize(c->stream));
     return GD_OK;
 }

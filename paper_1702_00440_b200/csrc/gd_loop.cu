@@ -552,7 +552,6 @@ __device__ __forceinline__ void gd_lp_commit(const gd_dev &d, const gd_lsm &sm, 
 __device__ __forceinline__ void gd_lp_correct_warp(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, int G, int p0, int pos, int p,
                                                    double t_next, int lane)
 {
-    const long long c0 = clock64();
     const int i = p0 + p;
     const double4 ad = GD_LP_AD(p, i), jk = GD_LP_JK(p, i);
     double s[6] = {0, 0, 0, 0, 0, 0};
@@ -574,13 +573,11 @@ __device__ __forceinline__ void gd_lp_correct_warp(const gd_dev &d, const gd_lsm
             s[3] += wgt * v[u][1].y; s[4] += wgt * v[u][2].x; s[5] += wgt * v[u][2].y;
         }
     }
-    const long long c0b = clock64() + (long long)(s[0] == 1e300);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
         for (int k = 0; k < 6; ++k) s[k] += __shfl_xor_sync(GD_FULL, s[k], o);
     }
-    const long long c1 = clock64();
     const double2 pxy = sm.pxy[p], pzm = sm.pzm[p], pvxy = sm.vxy[p];
     const double pvz = sm.vz[p];
     const int comp = lane < 2 ? lane : 2;
@@ -601,16 +598,9 @@ __device__ __forceinline__ void gd_lp_correct_warp(const gd_dev &d, const gd_lsm
     const double na1 = gd_norm3(s[0], s[1], s[2]), nj1 = gd_norm3(s[3], s[4], s[5]);
     const double na2 = gd_norm3(a2x, a2y, a2z), na3 = gd_norm3(a3x, a3y, a3z);
     r.dt = gd_new_step(na1, nj1, na2, na3, h, t_next, la.eta, la.dt_min, la.dt_max, la.halving_mode, r.flags);
-    const long long c2 = clock64();
     if (lane == 0) {
         const double a1v[3] = {s[0], s[1], s[2]}, j1v[3] = {s[3], s[4], s[5]};
         gd_lp_commit(d, sm, i, p, pzm.y, r, a1v, j1v, h, t_next);
-        if (blockIdx.x == 0 && threadIdx.x == 0) {
-            const long long c3 = clock64();
-            d.lp_ctl[13] += (unsigned long long)(c1 - c0);
-            d.lp_ctl[14] += (unsigned long long)(c2 - c1);
-            d.lp_ctl[15] += (unsigned long long)(c0b - c0);
-        }
     }
 }
 
