@@ -164,6 +164,14 @@ GD_API int gd_get_active(gd_ctx *ctx, int32_t *idx_dev, int64_t cap);
 /* Particle steps taken per level k (dt = 2^-k) since init -> counts_host[64]; and diagnostic counters
  * diag_host[2] = { time-step criteria that evaluated to NaN, clamps at dt_min }.  Synchronises. */
 GD_API int gd_get_level_histogram(gd_ctx *ctx, int64_t *counts_host, int64_t *diag_host);
+/* Lagrange radii, "the radii of spheres containing a certain mass fraction of the system" (Fig. 9, Fig. 11
+ * P:347): for each fraction f_k in (0, 1] (n_frac <= 16, HOST array) the radius, about the centre, of the smallest
+ * sphere that holds at least that fraction of the total mass, taken on the positions predicted to the current time
+ * -> radii_host[n_frac].  center_host: HOST {x, y, z}, or NULL = the centre of mass.  center_out_host: NULL or HOST
+ * [4] <- {centre x, y, z, total mass}.  Masses are counted in fixed point so that the result does not depend on the
+ * order of summation (R24).  On-device 8-pass radix select, no sort.  Synchronises. */
+GD_API int gd_lagrange_radii(gd_ctx *ctx, const double *center_host, const double *fractions_host, int n_frac,
+                             double *radii_host, double *center_out_host);
 /* Counters of the persistent block-step loop (k_block_loop, the kernel behind gd_step / gd_run_until that takes the
  * block steps) since init -> out_host[11] = { particle steps, block steps taken inside
  * the loop, ns spent inside it (device global timer, CTA 0), ns in its force phase, in the barrier after it, in its

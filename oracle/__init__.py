@@ -7,3 +7,4 @@ from .oracle import (  # noqa: F401
     HermiteOracle, build, pairsum, pairsum_longdouble, predict, correct, energy, next_block, block_init,
     block_update, initial_dt, num_threads, set_num_threads, DT_MAX, DT_MIN,
 )
+from . import lagrange  # noqa: F401,E402

@@ -51,6 +51,7 @@ SYMBOLS = {
     "gd_get_level_histogram": (_int, [_vp, _vp, _vp]),
     "gd_get_profile": (_int, [_vp, _vp]),
     "gd_get_loop_profile": (_int, [_vp, _vp]),
+    "gd_lagrange_radii": (_int, [_vp, _vp, _vp, _int, _vp, _vp]),
     "gd_fp64_peak_probe": (_int, [_int, _pdbl, _pdbl]),
 }
 
@@ -302,6 +303,15 @@ class Hermite:
         self._check(self._lib.gd_get_profile(self._h, p.ctypes.data))
         return {k: {"launches": int(p[4 * i]), "ms": float(p[4 * i + 1]), "pairs": float(p[4 * i + 2]),
                     "ms2": float(p[4 * i + 3])} for i, k in enumerate(("ipar", "jsplit", "ipar_small", "loop", "slice"))}
+
+    def lagrange_radii(self, fractions, center=None):
+        """Radii about `center` (None: the centre of mass) holding the given mass fractions -> (radii, centre[3], M)."""
+        f = np.ascontiguousarray(fractions, dtype=np.float64)
+        r, co = np.zeros(f.shape[0]), np.zeros(4)
+        c = None if center is None else np.ascontiguousarray(center, dtype=np.float64)
+        self._check(self._lib.gd_lagrange_radii(self._h, c.ctypes.data if c is not None else None, f.ctypes.data,
+                                                int(f.shape[0]), r.ctypes.data, co.ctypes.data))
+        return r, co[:3].copy(), float(co[3])
 
     def loop_profile(self) -> dict:
         o = np.zeros(11, dtype=np.int64)

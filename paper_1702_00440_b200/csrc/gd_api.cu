@@ -118,6 +118,7 @@ static size_t gd_carve(gd_dev *d, void *base, int64_t np, int64_t pcap)
     t.lp_L = w.take<double>(256);
     t.lp_cnt = w.take<int>(256);
     t.lp_ctl = w.take<unsigned long long>(16);
+    t.diag_scratch = w.take<unsigned long long>(4352);
     t.cell = w.take<double>(4);
     t.hist = w.take<long long>(64);
     t.diag = w.take<long long>(2);
@@ -374,6 +375,28 @@ extern "C" int gd_energy(gd_ctx *c, double *kinetic_host, double *potential_host
     GD_CUDA(c, cudaStreamSynchronize(c->stream));
     if (kinetic_host) *kinetic_host = c->h_cell[2];
     if (potential_host) *potential_host = c->h_cell[3];
+    return GD_OK;
+}
+
+extern "C" int gd_lagrange_radii(gd_ctx *c, const double *center_host, const double *fractions_host, int n_frac,
+                                 double *radii_host, double *center_out_host)
+{
+    if (!c || !fractions_host || !radii_host) return GD_EINVAL;
+    if (n_frac < 1 || n_frac > 16) return gd_fail(c, GD_EINVAL, "gd_lagrange_radii: 1 <= n_frac <= 16");
+    for (int k = 0; k < n_frac; ++k)
+        if (!(fractions_host[k] > 0.0 && fractions_host[k] <= 1.0)) return gd_fail(c, GD_EINVAL, "gd_lagrange_radii: fractions must lie in (0, 1]");
+    int rc = gdk_predict(c, c->t);
+    if (rc) return rc;
+    c->t_pred = c->t;
+    c->have_pred = true;
+    c->have_force = false;
+    double *st = (double *)c->d.staging;                     // [0, 16) fractions, [16, 32) radii (np >= 256: 7 np doubles)
+    GD_CUDA(c, cudaMemcpyAsync(st, fractions_host, n_frac * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    if ((rc = gdk_lagrange(c, center_host, st, n_frac, st + 16))) return rc;
+    GD_CUDA(c, cudaMemcpyAsync(radii_host, st + 16, n_frac * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    if (center_out_host)
+        GD_CUDA(c, cudaMemcpyAsync(center_out_host, c->d.diag_scratch, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
     return GD_OK;
 }
 

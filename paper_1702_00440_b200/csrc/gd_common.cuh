@@ -46,6 +46,7 @@ struct gd_dev {
     double *phi;                 // [np] per-particle potential sums  (energy)
     double *kin;                 // [np] per-particle kinetic terms   (energy)
     void *staging;               // [7 np] doubles: staging for host<->device copies of m, x, v
+    unsigned long long *diag_scratch;    // [4352] centre, scale, targets, prefixes and histograms of the Lagrange-radius select
     // persistent block-step loop (gd_loop.cu)
     double4 *lp_rec;             // [np + GD_LP_REC_SLACK][2] candidate records, one segment of S rows per CTA
     double *lp_L;                // [256] smallest t_i + dt_i of every CTA's slice
@@ -127,7 +128,8 @@ int gdk_loop(gd_ctx *c);
 int gdk_slice_setup(gd_ctx *c);
 int64_t gdk_slice_hi(const gd_ctx *c);
 int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out);
-int gdk_energy(gd_ctx *c);                                                                   // gd_energy.cu
+int gdk_energy(gd_ctx *c);
+int gdk_lagrange(gd_ctx *c, const double *center_host, const double *frac_dev, int n_frac, double *radii_dev);   // gd_diag.cu                                                                   // gd_energy.cu
 int gdk_fp64_probe(int iters, double *flops, double *ms);                                    // gd_probe.cu
 
 int gd_fail_cuda(gd_ctx *c, cudaError_t e, const char *what);

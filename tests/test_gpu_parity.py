@@ -462,3 +462,40 @@ def test_c2_energy_error_after_one_time_unit_matches_oracle(gd):
     err_ref = abs(gold["e1"] / gold["e0"] - 1.0)
     assert abs(k0 + u0 - gold["e0"]) <= 1e-13 * abs(gold["e0"])
     assert abs(err - err_ref) <= 0.1 * err_ref, (err, err_ref)
+
+
+# ------------------------------------------------------------------------------ diagnostics: Lagrange radii
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (2, 16384), (4, 6000), (5, 2047), (1, 3)])
+def test_lagrange_radii_match_oracle(gd, cfg, n):
+    from oracle import lagrange
+    w = W.config(cfg, n=n)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    fr = [0.005, 0.01, 0.02, 0.03, 0.04, 0.05, 0.06, 0.75, 0.90, 0.5, 1.0]    # Fig. 9 + half mass + all
+    r, c, mtot = h.lagrange_radii(fr)
+    r_ref, c_ref = lagrange.lagrange_radii(w.m, w.x, fr)
+    assert abs(mtot - w.m.sum()) <= 1e-14 * w.m.sum() and np.abs(c - c_ref).max() < 1e-14
+    # (C5's central particle sits on the centre of mass: its distance is the rounding noise of the centre)
+    assert np.all(np.abs(r - r_ref) <= 1e-12 * r_ref + 1e-14), (r, r_ref)
+    # about a given centre the centre drops out of the comparison: identical bits
+    r2, c2, _ = h.lagrange_radii(fr, center=[0.05, -0.1, 0.2])
+    r2_ref, _ = lagrange.lagrange_radii(w.m, w.x, fr, centre=[0.05, -0.1, 0.2])
+    assert np.array_equal(r2, r2_ref) and np.array_equal(c2, [0.05, -0.1, 0.2])
+    h.close()
+
+
+def test_lagrange_radii_follow_the_predicted_state_and_reject_bad_fractions(gd):
+    from oracle import lagrange
+    w = W.config(1)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    h.step(37)
+    for _ in range(37):
+        o.step()
+    xp, _ = oracle.predict(o.t, o.x, o.v, o.a, o.j, o.t_i)
+    r, _, _ = h.lagrange_radii([0.1, 0.5, 0.9])
+    r_ref, _ = lagrange.lagrange_radii(w.m, xp, [0.1, 0.5, 0.9])
+    assert np.abs(r / r_ref - 1.0).max() < 1e-11
+    for bad in ([0.0], [1.5], [float("nan")], list(np.linspace(0.01, 0.9, 17))):
+        with pytest.raises(gd.GravidyError):
+            h.lagrange_radii(bad)
+    h.close()
