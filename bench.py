@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--t-end", type=float, default=None, help="override the end time (experiments only)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the C3 force-kernel sweep (extra key)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-stages", action="store_true", help="skip the memory-bound stage timing at C5 size (extra key)")
     return ap.parse_args()
 
 
@@ -177,6 +178,64 @@ def force_sweep(gd, torch, W):
                      "frac_fp64_nominal": rate * FLOP_PER_PAIR / 1e12 / FP64_NOMINAL_TFLOPS})
     h.close()
     return {"workload": "C3 Plummer N=65536, back-to-back launches (state L2-resident)", "points": rows}
+
+
+def hbm_peak_gbs() -> tuple[float, str]:
+    """Measured copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the recipe's fallback."""
+    try:
+        return float(json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (burst)"
+    except (OSError, KeyError, ValueError):
+        return 6550.0, "fallback of /opt/skills/guides/B200_PROFILING.md"
+
+
+def stage_bandwidth(gd, torch, W):
+    """The memory-bound stages at C5's size, where the 193 MB state does not fit the
+    126 MB L2: next_block (16 B per particle), predictor (184 B per particle: 128 read + 56 written), corrector +
+    time step (340 B per active particle).  A shared step (dt_level_min = dt_level_max) makes every block step
+    all-active, so the corrector streams all N.  One warm-up step, then one step timed launch by launch with CUDA
+    events (extra key, not `value`)."""
+    w = W.config(5)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    peak, src = hbm_peak_gbs()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(fn, reps=1):
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            out = fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3 / reps, out
+
+    rows = {}
+    # the usual case first: the first block of C5 under its own block steps (a handful of active particles)
+    h.next_block()
+    s_nb, (_, n_first) = timed(h.next_block, 5)
+    rows["next_block"] = {"us": round(s_nb * 1e6, 2), "n_act": n_first, "algorithmic_bytes": 16.0 * w.n + 4.0 * n_first,
+                          "gbs": (16.0 * w.n + 4.0 * n_first) / s_nb / 1e9, "frac_hbm": (16.0 * w.n + 4.0 * n_first) / s_nb / 1e9 / peak,
+                          "note": "per call, including the device-to-host copy of (t_next, n_act) and the stream synchronisation"}
+    h.set_option("dt_level_min", 10)
+    h.set_option("dt_level_max", 10)
+    samples = {"next_block_all_active": [], "predictor": [], "corrector_timestep": []}
+    for step in range(4):                              # one warm-up step, three timed: the median is reported
+        s_nb, (t_next, n_act) = timed(h.next_block)
+        h.predict(t_next)
+        s_pr, _ = timed(lambda: h.predict(t_next), 10)
+        h.force_jerk(None)
+        s_co, _ = timed(h.correct_and_timestep)
+        assert n_act == w.n
+        if step:
+            for name, sec in zip(samples, (s_nb, s_pr, s_co)):
+                samples[name].append(sec)
+    for name, per in (("next_block_all_active", 20.0), ("predictor", 184.0), ("corrector_timestep", 340.0)):
+        sec, nbytes = statistics.median(samples[name]), per * w.n
+        rows[name] = {"us": round(sec * 1e6, 2), "algorithmic_bytes": nbytes, "gbs": nbytes / sec / 1e9,
+                      "frac_hbm": nbytes / sec / 1e9 / peak}
+    h.close()
+    rows["next_block_all_active"]["note"] = rows["next_block"]["note"] + "; 4 B of index written per active particle"
+    return {"workload": f"C5 size N={w.n}, shared step 2^-10 (all-active block steps), median of three steps after a warm-up step; "
+                        "predictor: 10 back-to-back launches", "hbm_peak_gbs": peak, "hbm_peak_source": src, "stages": rows}
 
 
 def cpu_sample_steps(n: int) -> int:
@@ -352,6 +411,8 @@ def finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, 
     }
     if not args.no_sweep:
         line["force_sweep"] = force_sweep(gd, torch, W)
+    if not args.no_stages:
+        line["memory_bound_stages"] = stage_bandwidth(gd, torch, W)
     if not args.no_cpu and world == 1:
         line["cpu_baseline"], _ = cpu_baseline(w, t_end)
     print(json.dumps(line), flush=True)

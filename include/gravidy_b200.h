@@ -87,9 +87,10 @@ GD_API const char *gd_last_error(const gd_ctx *ctx);
  * "halving_mode" (1: halve until dt <= dt_req [default]; 0: a single halving per step),
  * "slice_max_nact" (active sets up to this size go to k_force_slice, one CTA per SM over a shared-memory slice of
  * the sources, where the system is small enough for it; default 8192, 0 = off: the kernels above take over),
- * "loop_max_nact", "loop_small_nact", "loop_state_smem" (the persistent block-step loop behind gd_step /
- * gd_run_until: largest active set it takes [default: all], size up to which lanes stride over sources [96],
- * own state resident in shared memory [1]),
+ * "loop_max_nact", "loop_small_nact", "loop_state_smem", "loop_warp_correct" (the persistent block-step loop behind
+ * gd_step / gd_run_until: largest active set it takes [default: all], size up to which lanes stride over sources
+ * [96], own state resident in shared memory [1], number of own active particles up to which a CTA corrects them a
+ * warp each instead of a thread each [48]),
  * "profile" (0/1: time every force launch with CUDA events, see gd_get_profile).  GD_EINVAL on unknown keys. */
 GD_API int gd_set_option(gd_ctx *ctx, const char *key, double value);
 
@@ -194,6 +195,13 @@ GD_API int gd_get_profile(gd_ctx *ctx, double *prof_host);
  * achieved rate in flop/s (2 flop per FMA per lane) in *flops_host; ms_host receives the elapsed milliseconds.
  * Needs no ctx (it allocates and frees 8 bytes of device memory itself).  Synchronises the device. */
 GD_API int gd_fp64_peak_probe(int iters, double *flops_host, double *ms_host);
+
+/* Self-test of the device arithmetic: the predictor and corrector divide by the constants 6, 24, 120
+ * with a multiply and two FMAs instead of the division routine; the two must agree bit for bit.  Evaluates both on n
+ * random operands of the stream `seed` (all signs, binary exponents -960 .. 959, random significands) for each of
+ * the three constants and returns the number of differing results in *mismatches_host (0 = identical).  Needs no
+ * ctx; allocates and frees 8 bytes of device memory; synchronises the device. */
+GD_API int gd_selftest_div_const(int64_t n, uint64_t seed, int64_t *mismatches_host);
 
 #ifdef __cplusplus
 }

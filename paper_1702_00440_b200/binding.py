@@ -53,6 +53,7 @@ SYMBOLS = {
     "gd_get_loop_profile": (_int, [_vp, _vp]),
     "gd_lagrange_radii": (_int, [_vp, _vp, _vp, _int, _vp, _vp]),
     "gd_fp64_peak_probe": (_int, [_int, _pdbl, _pdbl]),
+    "gd_selftest_div_const": (_int, [C.c_int64, C.c_uint64, _vp]),
 }
 
 _lib = None
@@ -94,6 +95,15 @@ def fp64_peak_probe(iters: int = 1 << 15) -> tuple[float, float]:
     if rc:
         raise GravidyError(rc, "gd_fp64_peak_probe failed (no CUDA device?)")
     return f.value, ms.value
+
+
+def selftest_div_const(n: int = 1 << 24, seed: int = 1) -> int:
+    """Mismatches between the corrector's division by 6, 24, 120 (multiply + two FMAs) and x / c on n random operands."""
+    bad = C.c_int64(-1)
+    rc = load().gd_selftest_div_const(int(n), int(seed), C.byref(bad))
+    if rc:
+        raise GravidyError(rc, "gd_selftest_div_const failed (no CUDA device?)")
+    return int(bad.value)
 
 
 def _torch():

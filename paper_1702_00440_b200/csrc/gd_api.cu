@@ -181,6 +181,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->ipar_small_max_nact = 2048;
     c->loop_max_nact = (int64_t)1 << 40;      // every step the scratch allows
     c->loop_small_nact = 96;
+    c->loop_warp_correct = 48;
     c->slice_max_nact = 8192;
     c->loop_state_opt = 1;
     c->stream = (cudaStream_t)stream;
@@ -273,6 +274,7 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
         gd_graph_drop(c);
         return gdk_loop_setup(c);
     }
+    if (!strcmp(key, "loop_warp_correct")) { c->loop_warp_correct = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "profile")) {
         int rc = gd_prof_drain(c);
         c->profile = (int)value;
@@ -687,4 +689,13 @@ extern "C" int gd_fp64_peak_probe(int iters, double *flops_host, double *ms_host
 {
     if (iters < 1) return GD_EINVAL;
     return gdk_fp64_probe(iters, flops_host, ms_host) ? GD_ECUDA : GD_OK;
+}
+
+extern "C" int gd_selftest_div_const(int64_t n, uint64_t seed, int64_t *mismatches_host)
+{
+    if (n < 0 || !mismatches_host) return GD_EINVAL;
+    long long bad = 0;
+    if (gdk_selftest_div_const((long long)n, (unsigned long long)seed, &bad)) return GD_ECUDA;
+    *mismatches_host = (int64_t)bad;
+    return GD_OK;
 }

@@ -85,6 +85,7 @@ struct gd_ctx {
     int use_graph;
     int64_t loop_max_nact;               // option: largest active set the persistent loop takes (0 = loop off)
     int loop_state_opt;                  // option: keep the own state resident in shared memory when it fits
+    int64_t loop_warp_correct;           // option: a CTA owning up to this many active particles corrects them a warp each
     int64_t loop_small_nact;             // option: active sets up to this size use the lanes-over-sources mapping
     int loop_grid, loop_S, loop_hi, loop_cap, loop_state;   // geometry of k_block_loop (loop_grid = 0: not usable)
     size_t loop_smem;
@@ -130,6 +131,7 @@ int64_t gdk_slice_hi(const gd_ctx *c);
 int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out);
 int gdk_energy(gd_ctx *c);
 int gdk_lagrange(gd_ctx *c, const double *center_host, const double *frac_dev, int n_frac, double *radii_dev);   // gd_diag.cu                                                                   // gd_energy.cu
+int gdk_selftest_div_const(long long n, unsigned long long seed, long long *mismatches);          // gd_probe.cu
 int gdk_fp64_probe(int iters, double *flops, double *ms);                                    // gd_probe.cu
 
 int gd_fail_cuda(gd_ctx *c, cudaError_t e, const char *what);

@@ -11,6 +11,22 @@ __device__ __forceinline__ double gd_add(double a, double b) { return __dadd_rn(
 __device__ __forceinline__ double gd_sub(double a, double b) { return __dsub_rn(a, b); }
 __device__ __forceinline__ double gd_div(double a, double b) { return __ddiv_rn(a, b); }
 
+// x / C for the constants 6, 24, 120 of the predictor and corrector, correctly rounded without the division routine
+// (~35 dependent FP64 instructions): with y = RN(1/C), q = RN(x y) is within one ulp of x / C, r = x - q C is exact
+// (one FMA), and RN(q + r y) is the correctly rounded quotient (Markstein 1990: y correctly rounded, significand of C
+// not all ones).  Outside the range where neither r nor q r can underflow or overflow the division routine runs.
+// Bit for bit the result of x / C: gd_selftest_div_const compares the two on random operands.
+template <int C>
+__device__ __forceinline__ double gd_div_const(double x)
+{
+    constexpr double c = (double)C, y = 1.0 / (double)C;
+    const double ax = fabs(x);
+    if (!(ax > 0x1p-900 && ax < 0x1p900)) return __ddiv_rn(x, c);
+    const double q = __dmul_rn(x, y);
+    const double r = __fma_rn(-q, c, x);
+    return __fma_rn(r, y, q);
+}
+
 // ---- predictor: D = t - t_i ; xp = x + v D + a D^2/2 + jerk D^3/6 ; vp = v + a D + jerk D^2/2 -------------------
 struct gd_pred { double x, y, z, vx, vy, vz; };
 
@@ -19,7 +35,7 @@ __device__ __forceinline__ gd_pred gd_predict_record(const double4 &xm, const do
     double D = gd_sub(t, vt.w);
     double DD = gd_mul(D, D);
     double D2 = gd_mul(DD, 0.5);                              // = DD / 2 exactly
-    double D3 = gd_div(gd_mul(DD, D), 6.0);
+    double D3 = gd_div_const<6>(gd_mul(DD, D));
 #define GD_PX(x0, v0, a0, j0) gd_add(gd_add(gd_add((x0), gd_mul((v0), D)), gd_mul((a0), D2)), gd_mul((j0), D3))
 #define GD_PV(v0, a0, j0) gd_add(gd_add((v0), gd_mul((a0), D)), gd_mul((j0), D2))
     gd_pred p;
@@ -69,8 +85,8 @@ __device__ __forceinline__ gd_corr1 gd_correct_component(double xp, double vp, d
     double a3 = p.pow2 ? gd_mul(n3, p.ih3) : gd_div(n3, p.h3);
     gd_corr1 r;
     // x = xp + a2 h^4/24 + a3 h^5/120 ;  v = vp + a2 h^3/6 + a3 h^4/24
-    r.xnew = gd_add(gd_add(xp, gd_div(gd_mul(a2, p.h4), 24.0)), gd_div(gd_mul(a3, p.h5), 120.0));
-    r.vnew = gd_add(gd_add(vp, gd_div(gd_mul(a2, p.h3), 6.0)), gd_div(gd_mul(a3, p.h4), 24.0));
+    r.xnew = gd_add(gd_add(xp, gd_div_const<24>(gd_mul(a2, p.h4))), gd_div_const<120>(gd_mul(a3, p.h5)));
+    r.vnew = gd_add(gd_add(vp, gd_div_const<6>(gd_mul(a2, p.h3))), gd_div_const<24>(gd_mul(a3, p.h4)));
     r.a2e = gd_add(a2, gd_mul(h, a3));        // second derivative at the end of the step
     r.a3 = a3;
     return r;

@@ -40,6 +40,7 @@ struct gd_largs {
     int hi;                          // largest active set the loop takes
     int cap;                         // positions the partial-sum scratch holds: partial[cap][G][6]
     int small_hi;                    // n_act <= small_hi: lanes over sources; above: lanes over sinks
+    int wc_hi;                       // [correct]: up to wc_hi own active particles a warp each, above a thread each
     int state;                       // != 0: the own state is resident in shared memory
     double eps2, eta, dt_min, dt_max;
     int halving_mode;
@@ -755,7 +756,7 @@ k_block_loop(gd_dev d, gd_largs la)
             const unsigned long long o0 = gd_gtime();
             const int pre = sm.spre[me];
             // few own active particles: a warp each (lanes over the CTAs' partial sums); many: a thread each
-            if (cnt_me <= 2 * GD_LP_WARPS) {
+            if (cnt_me <= la.wc_hi) {
                 for (int k = warp; k < cnt_me; k += GD_LP_WARPS) gd_lp_correct_warp(d, sm, la, G, p0, pre + k, sm.lact[k], t_next, lane);
             } else {
                 for (int k = tid; k < cnt_me; k += GD_LP_THREADS) gd_lp_correct_thread(d, sm, la, G, p0, pre + k, sm.lact[k], t_next);
@@ -959,6 +960,7 @@ int gdk_loop(gd_ctx *c)
     la.state = c->loop_state;
     int64_t sh = c->loop_small_nact < GD_LP_MAX_SMALL ? c->loop_small_nact : GD_LP_MAX_SMALL;
     la.small_hi = (int)(sh < 0 ? 0 : sh);
+    la.wc_hi = (int)(c->loop_warp_correct < 0 ? 0 : (c->loop_warp_correct > 4096 ? 4096 : c->loop_warp_correct));
     la.eps2 = c->eps2;
     la.eta = c->eta;
     la.dt_min = c->dt_min;
@@ -1013,6 +1015,7 @@ int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out,
     la.cap = (int)((n_act + 31) / 32 * 32);
     int64_t sh = c->loop_small_nact < GD_LP_MAX_SMALL ? c->loop_small_nact : GD_LP_MAX_SMALL;
     la.small_hi = (int)(sh < 0 ? 0 : sh);
+    la.wc_hi = (int)(c->loop_warp_correct < 0 ? 0 : (c->loop_warp_correct > 4096 ? 4096 : c->loop_warp_correct));
     la.state = 0;
     la.eps2 = c->eps2;
     la.eta = c->eta;

@@ -92,7 +92,10 @@ k_block_compact(gd_dev d, int64_t np, int per_block, int dev)
     const double t_next = d.cell[0];
     const int64_t begin = (int64_t)bid * per_block;
     const int64_t end = min(np, begin + per_block);
-    const int rounds = (int)((end - begin + GD_SCAN_THREADS - 1) / GD_SCAN_THREADS);
+    // k_block_min left the minimum of this very range in blockmin[bid] (same geometry): a range whose minimum is not
+    // t_next holds no active particle and is not read again -- under block time steps that is almost every range
+    const bool any = __ldcg(d.blockmin + bid) == t_next;
+    const int rounds = any ? (int)((end - begin + GD_SCAN_THREADS - 1) / GD_SCAN_THREADS) : 0;
 
     // pass 1: flags and per-round counts
     unsigned int mask = 0;

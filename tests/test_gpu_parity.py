@@ -118,6 +118,13 @@ def test_force_unsorted_and_repeated_indices(gd):
 
 
 # ------------------------------------------------------------------------------ init, predictor, corrector
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_division_by_constants_is_the_correctly_rounded_quotient(gd, seed):
+    # gd_div_const (x / 6, x / 24, x / 120 as a multiply and two FMAs) against the division routine, bit for bit,
+    # on 2^26 random operands per constant; the oracle divides (oracle/hermite_oracle.c), so must the device
+    assert gd.selftest_div_const(1 << 26, seed) == 0
+
+
 def test_init_matches_oracle(gd):
     w = W.config(1)
     h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
