@@ -53,6 +53,7 @@ def parse_args():
     ap.add_argument("--no-sweep", action="store_true", help="skip the C3 force-kernel sweep (extra key)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-stages", action="store_true", help="skip the memory-bound stage timing at C5 size (extra key)")
+    ap.add_argument("--only-stages", action="store_true", help="run only the memory-bound stage timing (for ncu captures)")
     return ap.parse_args()
 
 
@@ -287,6 +288,9 @@ def main_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_1702_00440_b200 import binding as gd, workloads as W
     gd.load()
+    if args.only_stages:
+        print(json.dumps({"memory_bound_stages": stage_bandwidth(gd, torch, W)}), flush=True)
+        return
     w, t_end = load_workload(args)
 
     # device-resident and pinned-host copies of the inputs

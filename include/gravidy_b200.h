@@ -86,7 +86,8 @@ GD_API const char *gd_last_error(const gd_ctx *ctx);
  * "dt_level_min", "dt_level_max" (override GD_LEVEL_MIN/MAX before the first step; 0 <= min <= max <= 52),
  * "halving_mode" (1: halve until dt <= dt_req [default]; 0: a single halving per step),
  * "slice_max_nact" (active sets up to this size go to k_force_slice, one CTA per SM over a shared-memory slice of
- * the sources, where the system is small enough for it; default 8192, 0 = off: the kernels above take over),
+ * the sources; default 8192, 0 = off: the kernels above take over), "slice_passes" (slices per CTA of that kernel:
+ * 0 = the fewest whose records fit in shared memory [default: 1 up to N ~ 3.5e5, 3 at C5's size], 1..16 forces a count),
  * "loop_max_nact", "loop_small_nact", "loop_state_smem", "loop_warp_correct" (the persistent block-step loop behind
  * gd_step / gd_run_until: largest active set it takes [default: all], size up to which lanes stride over sources
  * [96], own state resident in shared memory [1], number of own active particles up to which a CTA corrects them a

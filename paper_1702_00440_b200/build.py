@@ -39,7 +39,7 @@ def build_library(force: bool = False, verbose: bool = False) -> Path:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB.with_suffix(f".tmp{os.getpid()}.so")
-    cmd = [nvcc, *NVCC_FLAGS, "-shared", "-I", str(INCLUDE), "-o", str(tmp), *map(str, sources())]
+    cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("GD_NVCC_EXTRA", "").split(), "-shared", "-I", str(INCLUDE), "-o", str(tmp), *map(str, sources())]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.run(cmd, check=True)

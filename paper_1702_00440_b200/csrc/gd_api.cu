@@ -183,6 +183,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->loop_small_nact = 96;
     c->loop_warp_correct = 48;
     c->slice_max_nact = 8192;
+    c->slice_passes_opt = 0;
     c->loop_state_opt = 1;
     c->stream = (cudaStream_t)stream;
     gd_carve(&c->d, ws, c->np, c->pcap);
@@ -266,7 +267,13 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
     if (!strcmp(key, "jsplit_max_nact")) { c->jsplit_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "ipar_small_max_nact")) { c->ipar_small_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "use_graph")) { c->use_graph = value != 0.0; return GD_OK; }
-    if (!strcmp(key, "slice_max_nact")) { c->slice_max_nact = (int64_t)value; return GD_OK; }
+    if (!strcmp(key, "slice_max_nact")) { c->slice_max_nact = (int64_t)value; gd_graph_drop(c); return GD_OK; }
+    if (!strcmp(key, "slice_passes")) {
+        if (value < 0 || value > 16) return gd_fail(c, GD_EINVAL, "gd_set_option: slice_passes out of range");
+        c->slice_passes_opt = (int64_t)value;
+        gd_graph_drop(c);
+        return gdk_slice_setup(c);
+    }
     if (!strcmp(key, "loop_max_nact") || !strcmp(key, "loop_small_nact") || !strcmp(key, "loop_state_smem")) {
         if (!strcmp(key, "loop_max_nact")) c->loop_max_nact = (int64_t)value;
         else if (!strcmp(key, "loop_small_nact")) c->loop_small_nact = (int64_t)value;

@@ -90,7 +90,8 @@ struct gd_ctx {
     int loop_grid, loop_S, loop_hi, loop_cap, loop_state;   // geometry of k_block_loop (loop_grid = 0: not usable)
     size_t loop_smem;
     int64_t slice_max_nact;              // option: largest active set gd_force_jerk gives to k_force_slice (0 = off)
-    int slice_grid, slice_S;             // geometry of k_force_slice (slice_grid = 0: not usable)
+    int slice_grid, slice_S, slice_passes;   // geometry of k_force_slice (slice_grid = 0: not usable)
+    int64_t slice_passes_opt;            // option: slices per CTA (0 = the fewest that fit shared memory)
     size_t slice_smem;
     int64_t graph_nodes;                 // kernel nodes in step_graph
     int sm_count;
@@ -128,7 +129,7 @@ int gdk_loop_setup(gd_ctx *c);                                                  
 int gdk_loop(gd_ctx *c);
 int gdk_slice_setup(gd_ctx *c);
 int64_t gdk_slice_hi(const gd_ctx *c);
-int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out);
+int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out, bool dev);
 int gdk_energy(gd_ctx *c);
 int gdk_lagrange(gd_ctx *c, const double *center_host, const double *frac_dev, int n_frac, double *radii_dev);   // gd_diag.cu                                                                   // gd_energy.cu
 int gdk_selftest_div_const(long long n, unsigned long long seed, long long *mismatches);          // gd_probe.cu

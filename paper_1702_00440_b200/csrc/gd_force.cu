@@ -27,6 +27,19 @@ namespace cg = cooperative_groups;
 
 #define GD_STAGES 2
 #define GD_IPAR_THREADS 128
+// the large-set i-parallel kernel: sinks per thread, resident CTAs per SM it is compiled for (register budget), and
+// the unrolling of its source loop -- tuning knobs (measured on B200: see DESIGN.md section 5)
+#ifndef GD_L_BI
+#define GD_L_BI 2
+#endif
+#ifndef GD_IPAR_L_CTAS
+#define GD_IPAR_L_CTAS 3
+#endif
+#ifndef GD_IPAR_UNROLL
+#define GD_IPAR_UNROLL 2
+#endif
+#define GD_PRAGMA_(x) _Pragma(#x)
+#define GD_PRAGMA_UNROLL(n) GD_PRAGMA_(unroll n)
 #define GD_JS_THREADS 256
 #define GD_JS_WARPS (GD_JS_THREADS / 32)
 #define GD_JS_CLUSTER 8
@@ -116,7 +129,7 @@ __device__ __forceinline__ int gd_active_count(const gd_fargs &fa)
 // otherwise partial[split][k][6], and the LAST unit of an i-tile to finish (ticket) sums the splits in a fixed
 // order -- whoever does it.
 template <int BI, int WJ, bool EPS0>
-__global__ void __launch_bounds__(GD_IPAR_THREADS, (BI == 1 ? 7 : 5))
+__global__ void __launch_bounds__(GD_IPAR_THREADS, (BI == 1 ? 7 : GD_IPAR_L_CTAS))
 k_force_ipar(gd_dev d, gd_fargs fa)
 {
     constexpr int WI = 4 / WJ;
@@ -182,7 +195,7 @@ k_force_ipar(gd_dev d, gd_fargs fa)
             const gd_tile &T = tile[s];
             const int per = cnt / WJ;
             const int jb = wj * per, je = jb + per;
-#pragma unroll 2
+            GD_PRAGMA_UNROLL(GD_IPAR_UNROLL)
             for (int jj = jb; jj < je; ++jj) {
                 double2 xy = T.pxy[jj], zm = T.pzm[jj], vxy = T.vxy[jj];
                 gd_src sj{xy.x, xy.y, zm.x, zm.y, vxy.x, vxy.y, T.vz[jj]};
@@ -449,7 +462,7 @@ k_force_jsplit(gd_dev d, gd_fargs fa)
 //   i-parallel S   js_hi < n_act <= ipar_s_hi      k_force_ipar<1, 4> (i-tile of 32 sinks), persistent grid
 //   i-parallel L   ipar_s_hi < n_act               k_force_ipar<2, 1> (i-tile of 256 sinks), persistent grid
 #define GD_TI_S 32
-#define GD_TI_L 256
+#define GD_TI_L (128 * GD_L_BI)
 
 // Cost of covering i_tiles i-tiles with s source splits, in SM cycles: work units are dealt evenly to the SMs, an
 // SM's FP64 pipe (64 lanes) is shared by the units it holds, a unit's start-up latency overlaps with the other
@@ -492,7 +505,7 @@ int gdk_force_setup(gd_ctx *c)
     const int n_units = (int)(c->np / GD_UNIT_J);
     int res_s = 0, res_l = 0;
     GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&res_s, k_force_ipar<1, 4, false>, GD_IPAR_THREADS, 0));
-    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&res_l, k_force_ipar<2, 1, false>, GD_IPAR_THREADS, 0));
+    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&res_l, k_force_ipar<GD_L_BI, 1, false>, GD_IPAR_THREADS, 0));
     if (res_s < 1) res_s = 1;
     if (res_l < 1) res_l = 1;
     c->grid_s = c->sm_count * res_s;
@@ -506,7 +519,7 @@ int gdk_force_setup(gd_ctx *c)
     c->h_geom_l = (int *)malloc(sizeof(int2) * (size_t)(tiles_l + 1));
     if (!c->h_geom_s || !c->h_geom_l) return gd_fail_cuda(c, cudaErrorMemoryAllocation, "gdk_force_setup");
     gd_fill_geom((int2 *)c->h_geom_s, tiles_s, n_units, c->pcap, c->sm_count, res_s, 1, GD_TI_S, true);
-    gd_fill_geom((int2 *)c->h_geom_l, tiles_l, n_units, c->pcap, c->sm_count, res_l, 2, GD_TI_L, false);
+    gd_fill_geom((int2 *)c->h_geom_l, tiles_l, n_units, c->pcap, c->sm_count, res_l, GD_L_BI, GD_TI_L, false);
     // the host copies stay alive in the context, so the copies need no synchronisation here
     GD_CUDA(c, cudaMemcpyAsync(c->d.geom_s, c->h_geom_s, sizeof(int2) * (size_t)(tiles_s + 1), cudaMemcpyHostToDevice, c->stream));
     GD_CUDA(c, cudaMemcpyAsync(c->d.geom_l, c->h_geom_l, sizeof(int2) * (size_t)(tiles_l + 1), cudaMemcpyHostToDevice, c->stream));
@@ -586,8 +599,8 @@ int gdk_force(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, doubl
     const int slot = gd_prof_begin(c);
     int rc;
     if (kind == 4) {
-        rc = gdk_force_slice(c, idx, n_act, a_out, j_out);
-        c->last_geom[0] = 4; c->last_geom[1] = c->slice_grid; c->last_geom[2] = c->slice_S; c->last_geom[3] = 0;
+        rc = gdk_force_slice(c, idx, n_act, a_out, j_out, false);
+        c->last_geom[0] = 4; c->last_geom[1] = c->slice_grid; c->last_geom[2] = c->slice_S; c->last_geom[3] = c->slice_passes;
     } else if (kind == 1) {
         int64_t i_tiles = (n_act + 31) / 32;
         rc = gd_launch_jsplit(c, gd_make_fargs(c, idx, n_act, false, 0, INT_MAX, nullptr, a_out, j_out), c->js_clusters);
@@ -600,7 +613,7 @@ int gdk_force(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, doubl
     } else {
         int64_t i_tiles = (n_act + GD_TI_L - 1) / GD_TI_L;
         int grid = (int)(i_tiles * 1024 < c->grid_l ? i_tiles * 1024 : c->grid_l);
-        rc = gd_launch_ipar<2, 1>(c, gd_make_fargs(c, idx, n_act, false, 0, INT_MAX, c->d.geom_l, a_out, j_out), grid);
+        rc = gd_launch_ipar<GD_L_BI, 1>(c, gd_make_fargs(c, idx, n_act, false, 0, INT_MAX, c->d.geom_l, a_out, j_out), grid);
         c->last_geom[0] = 0; c->last_geom[1] = (int)i_tiles; c->last_geom[2] = c->h_geom_l[2 * i_tiles]; c->last_geom[3] = c->h_geom_l[2 * i_tiles + 1];
     }
     c->last_force_kernel = kind == 4 ? 4 : (kind == 1 ? 2 : (kind == 2 ? 3 : 1));
@@ -613,11 +626,19 @@ int gdk_force_dev(gd_ctx *c)
 {
     const int js_hi = gd_js_hi(c), s_hi = gd_s_hi(c);
     int rc = 0;
-    if (js_hi > 0)
-        rc = gd_launch_jsplit(c, gd_make_fargs(c, c->d.idx, 0, true, 0, js_hi, nullptr, c->d.a1, c->d.j1), c->js_clusters);
-    if (!rc && s_hi > js_hi)
-        rc = gd_launch_ipar<1, 4>(c, gd_make_fargs(c, c->d.idx, 0, true, js_hi, s_hi, c->d.geom_s, c->d.a1, c->d.j1), c->grid_s);
-    if (!rc && s_hi < c->np)
-        rc = gd_launch_ipar<2, 1>(c, gd_make_fargs(c, c->d.idx, 0, true, s_hi, INT_MAX, c->d.geom_l, c->d.a1, c->d.j1), c->grid_l);
+    // the same ranges as gdk_force: k_force_slice (kernel + fold, both reading the count on the device) takes the
+    // active sets up to its limit, the kernels behind it start above `lo`
+    int lo = (int)gdk_slice_hi(c);
+    if (lo > 0) rc = gdk_force_slice(c, c->d.idx, lo, c->d.a1, c->d.j1, true);
+    if (!rc && js_hi > lo) {
+        rc = gd_launch_jsplit(c, gd_make_fargs(c, c->d.idx, 0, true, lo, js_hi, nullptr, c->d.a1, c->d.j1), c->js_clusters);
+        lo = js_hi;
+    }
+    if (!rc && s_hi > lo) {
+        rc = gd_launch_ipar<1, 4>(c, gd_make_fargs(c, c->d.idx, 0, true, lo, s_hi, c->d.geom_s, c->d.a1, c->d.j1), c->grid_s);
+        lo = s_hi;
+    }
+    if (!rc && lo < c->np)
+        rc = gd_launch_ipar<GD_L_BI, 1>(c, gd_make_fargs(c, c->d.idx, 0, true, lo, INT_MAX, c->d.geom_l, c->d.a1, c->d.j1), c->grid_l);
     return rc;
 }

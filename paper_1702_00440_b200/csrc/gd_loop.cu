@@ -44,6 +44,7 @@ struct gd_largs {
     int state;                       // != 0: the own state is resident in shared memory
     double eps2, eta, dt_min, dt_max;
     int halving_mode;
+    int passes;                      // k_force_slice: slices per CTA, taken one after the other (1 where n / grid records fit)
     int ext;                         // != 0 (k_force_slice): the sinks are named by ext_idx in the predicted planes
     const int32_t *ext_idx;          //   (NULL: sink k = particle k); 0 (k_block_loop): they are the published records
 };
@@ -801,12 +802,28 @@ k_block_loop(gd_dev d, gd_largs la)
 // evaluates the partial sums of EVERY listed sink against it, with the mappings above.  The partial rows are folded
 //   n_act <= 16:  by the last CTA to finish (ticket), a warp per sink over the G contiguous rows of its position;
 //   larger:       by k_fold_slice_warp, the same with a warp per sink over the whole machine (one coalesced read each).
+// Systems whose 1/G of the source records does not fit in shared memory (C5: 7085 records per SM) are cut into
+// T = P G slices instead and CTA c takes the slices c, G + c, ... one after the other (P passes, T partial rows per
+// sink): the sinks stay in place, only the slice is reloaded.
+// Device-count form (n_act_dev != NULL: the captured block-step graph of systems too large for the persistent loop):
+// the active count is read from device memory and the kernel runs only for lo < n_act <= hi.
 #define GD_SL_TICKET_MAX 16
+#define GD_SL_MAX_PASSES 16
 struct gd_sargs {
     int n_act;
     double *a_out, *j_out;           // [n_act,3]
     unsigned int *ticket;
+    const long long *n_act_dev;
+    int lo, hi;
 };
+
+__device__ __forceinline__ bool gd_slice_count(const gd_sargs &sa, int &n_act)
+{
+    n_act = sa.n_act;
+    if (!sa.n_act_dev) return true;
+    n_act = (int)__ldcg(sa.n_act_dev);
+    return n_act > sa.lo && n_act <= sa.hi;
+}
 
 template <bool EPS0>
 __global__ void __launch_bounds__(GD_LP_THREADS, 1)
@@ -816,19 +833,10 @@ k_force_slice(gd_dev d, gd_largs la, gd_sargs sa)
     __shared__ bool s_last;
     const gd_lsm sm = gd_lsm_carve(gd_lp_smem, la.S, 0);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int G = gridDim.x, me = blockIdx.x;
-    const int n_act = sa.n_act;
-    const int p0 = gd_slice_begin(me, la.n, G);
-    const int cnt_own = gd_slice_begin(me + 1, la.n, G) - p0;
-    const int rounds = (cnt_own + 31) / 32;
+    const int G = gridDim.x, me = blockIdx.x, T = G * la.passes;
+    int n_act;
+    if (!gd_slice_count(sa, n_act)) return;
     const bool small = n_act <= la.small_hi;
-    for (int p = tid; p < rounds * 32; p += GD_LP_THREADS) {
-        const bool in = p < cnt_own;
-        sm.pxy[p] = in ? d.pxy[p0 + p] : make_double2(0.0, 0.0);
-        sm.pzm[p] = in ? d.pzm[p0 + p] : make_double2(0.0, 0.0);
-        sm.vxy[p] = in ? d.vxy[p0 + p] : make_double2(0.0, 0.0);
-        sm.vz[p] = in ? d.vz[p0 + p] : 0.0;
-    }
     if (small) {
         for (int e = tid; e < 4 * n_act; e += GD_LP_THREADS) {
             const int pos = e >> 2, part = e & 3;
@@ -841,11 +849,25 @@ k_force_slice(gd_dev d, gd_largs la, gd_sargs sa)
             sm.sink[e] = v;
         }
     }
-    __syncthreads();
-    const size_t ps = (size_t)6 * G;
-    double *out = d.partial + (size_t)me * 6;
-    if (small) gd_lp_force_small<EPS0>(d, sm, la, out, (int)ps, n_act, rounds);
-    else gd_lp_force_big<EPS0>(d, sm, la, out, (int)ps, G, n_act, cnt_own);
+    const size_t ps = (size_t)6 * T;
+    for (int pass = 0; pass < la.passes; ++pass) {
+        const int sl = pass * G + me;
+        const int p0 = gd_slice_begin(sl, la.n, T);
+        const int cnt_own = gd_slice_begin(sl + 1, la.n, T) - p0;
+        const int rounds = (cnt_own + 31) / 32;
+        if (pass) __syncthreads();                           // every warp is done with the previous slice
+        for (int p = tid; p < rounds * 32; p += GD_LP_THREADS) {
+            const bool in = p < cnt_own;
+            sm.pxy[p] = in ? d.pxy[p0 + p] : make_double2(0.0, 0.0);
+            sm.pzm[p] = in ? d.pzm[p0 + p] : make_double2(0.0, 0.0);
+            sm.vxy[p] = in ? d.vxy[p0 + p] : make_double2(0.0, 0.0);
+            sm.vz[p] = in ? d.vz[p0 + p] : 0.0;
+        }
+        __syncthreads();
+        double *out = d.partial + (size_t)sl * 6;
+        if (small) gd_lp_force_small<EPS0>(d, sm, la, out, (int)ps, n_act, rounds);
+        else gd_lp_force_big<EPS0>(d, sm, la, out, (int)ps, T, n_act, cnt_own);
+    }
     if (n_act > GD_SL_TICKET_MAX) return;
 
     // a handful of sinks: the last CTA to arrive folds; a warp per sink, lanes over the G contiguous rows of its position
@@ -862,7 +884,7 @@ k_force_slice(gd_dev d, gd_largs la, gd_sargs sa)
     for (int pos = warp; pos < n_act; pos += GD_LP_WARPS) {
         const double *base = d.partial + (size_t)pos * ps;
         double s[6] = {0, 0, 0, 0, 0, 0};
-        for (int c = lane; c < G; c += 32) {
+        for (int c = lane; c < T; c += 32) {
             const double2 *row = reinterpret_cast<const double2 *>(base + (size_t)c * 6);
             const double2 u0 = __ldcg(row), u1 = __ldcg(row + 1), u2 = __ldcg(row + 2);
             s[0] += u0.x; s[1] += u0.y; s[2] += u1.x; s[3] += u1.y; s[4] += u2.x; s[5] += u2.y;
@@ -879,26 +901,32 @@ k_force_slice(gd_dev d, gd_largs la, gd_sargs sa)
     }
 }
 
-// partial[pos][c][6] -> a_out, j_out; one warp per sink: lanes stride over the G contiguous rows, fixed butterfly
+// partial[pos][c][6] -> a_out, j_out; one warp per sink: lanes stride over the G contiguous rows (G = slices: CTAs x
+// passes), GD_LP_MAX_GRID rows in flight at a time, fixed butterfly
 __global__ void __launch_bounds__(GD_LP_THREADS)
 k_fold_slice_warp(gd_dev d, int G, gd_sargs sa)
 {
     const int lane = threadIdx.x & 31, pos = blockIdx.x * GD_LP_WARPS + (threadIdx.x >> 5);
-    if (pos >= sa.n_act) return;
+    int n_act;
+    if (!gd_slice_count(sa, n_act)) return;
+    if (sa.n_act_dev && n_act <= GD_SL_TICKET_MAX) return;   // folded inside k_force_slice
+    if (pos >= n_act) return;
     const double2 *base = reinterpret_cast<const double2 *>(d.partial + (size_t)pos * 6 * G);
-    double2 v[GD_LP_MAX_GRID / 32][3];
-#pragma unroll
-    for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
-        const int c = lane + 32 * u;
-        const double2 *row = base + 3 * (c < G ? c : lane);
-        v[u][0] = __ldcg(row); v[u][1] = __ldcg(row + 1); v[u][2] = __ldcg(row + 2);
-    }
     double s[6] = {0, 0, 0, 0, 0, 0};
+    for (int c0 = 0; c0 < G; c0 += GD_LP_MAX_GRID) {
+        double2 v[GD_LP_MAX_GRID / 32][3];
 #pragma unroll
-    for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
-        const double wgt = (lane + 32 * u < G) ? 1.0 : 0.0;
-        s[0] += wgt * v[u][0].x; s[1] += wgt * v[u][0].y; s[2] += wgt * v[u][1].x;
-        s[3] += wgt * v[u][1].y; s[4] += wgt * v[u][2].x; s[5] += wgt * v[u][2].y;
+        for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
+            const int c = c0 + lane + 32 * u;
+            const double2 *row = base + 3 * (c < G ? c : lane);
+            v[u][0] = __ldcg(row); v[u][1] = __ldcg(row + 1); v[u][2] = __ldcg(row + 2);
+        }
+#pragma unroll
+        for (int u = 0; u < GD_LP_MAX_GRID / 32; ++u) {
+            const double wgt = (c0 + lane + 32 * u < G) ? 1.0 : 0.0;
+            s[0] += wgt * v[u][0].x; s[1] += wgt * v[u][0].y; s[2] += wgt * v[u][1].x;
+            s[3] += wgt * v[u][1].y; s[4] += wgt * v[u][2].x; s[5] += wgt * v[u][2].y;
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -966,6 +994,7 @@ int gdk_loop(gd_ctx *c)
     la.dt_min = c->dt_min;
     la.dt_max = c->dt_max;
     la.halving_mode = c->halving_mode;
+    la.passes = 1;
     la.ext = 0;
     la.ext_idx = nullptr;
     void *args[] = {(void *)&c->d, (void *)&la};
@@ -982,16 +1011,24 @@ int gdk_slice_setup(gd_ctx *c)
     c->slice_grid = 0;
     int grid = c->sm_count < GD_LP_MAX_GRID ? c->sm_count : GD_LP_MAX_GRID;
     if (grid < 1 || c->n > INT_MAX / 2) return 0;
-    int64_t S = (c->n + grid - 1) / grid;
-    S = (S + 31) / 32 * 32;
     int dev = 0, max_smem = 0;
     GD_CUDA(c, cudaGetDevice(&dev));
     GD_CUDA(c, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-    const size_t bytes = gd_lsm_bytes((int)S, 0);
-    if (bytes > (size_t)max_smem) return 0;
+    // passes: the fewest slices per CTA whose records fit in shared memory (option `slice_passes` forces a count)
+    int64_t S = 0;
+    size_t bytes = 0;
+    int passes = c->slice_passes_opt > 0 ? (int)c->slice_passes_opt : 1;
+    for (;; ++passes) {
+        S = (c->n + (int64_t)grid * passes - 1) / ((int64_t)grid * passes);
+        S = (S + 31) / 32 * 32;
+        bytes = gd_lsm_bytes((int)S, 0);
+        if (bytes <= (size_t)max_smem) break;
+        if (c->slice_passes_opt > 0 || passes >= GD_SL_MAX_PASSES) return 0;
+    }
     GD_CUDA(c, cudaFuncSetAttribute(k_force_slice<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     GD_CUDA(c, cudaFuncSetAttribute(k_force_slice<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     c->slice_grid = grid;
+    c->slice_passes = passes;
     c->slice_S = (int)S;
     c->slice_smem = bytes;
     return 0;
@@ -1002,15 +1039,18 @@ int64_t gdk_slice_hi(const gd_ctx *c)
 {
     if (c->slice_grid < 1) return 0;
     int64_t hi = c->slice_max_nact < c->np ? c->slice_max_nact : c->np;
-    const int64_t cap = c->pcap / c->slice_grid / 32 * 32;
+    const int64_t cap = c->pcap / ((int64_t)c->slice_grid * c->slice_passes) / 32 * 32;
     return hi < cap ? hi : cap;
 }
 
-int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out)
+// dev = false: the host knows n_act (explicit call).  dev = true (captured graph): the count is read from device memory
+// (cell[1]) and the kernels run only for 0 < n_act <= n_act (the argument is then the largest set they take).
+int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out, bool dev)
 {
     gd_largs la;
     la.n = (int)c->n;
     la.S = c->slice_S;
+    la.passes = c->slice_passes;
     la.hi = (int)n_act;
     la.cap = (int)((n_act + 31) / 32 * 32);
     int64_t sh = c->loop_small_nact < GD_LP_MAX_SMALL ? c->loop_small_nact : GD_LP_MAX_SMALL;
@@ -1029,13 +1069,16 @@ int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out,
     sa.a_out = a_out;
     sa.j_out = j_out;
     sa.ticket = c->d.work + 2;
+    sa.n_act_dev = dev ? (const long long *)c->d.cell + 1 : nullptr;
+    sa.lo = 0;
+    sa.hi = (int)n_act;
     if (c->eps2 < 2.3e-308)
         k_force_slice<true><<<c->slice_grid, GD_LP_THREADS, c->slice_smem, c->stream>>>(c->d, la, sa);
     else
         k_force_slice<false><<<c->slice_grid, GD_LP_THREADS, c->slice_smem, c->stream>>>(c->d, la, sa);
     GD_LAUNCH_CHECK(c, "k_force_slice");
     if (n_act > GD_SL_TICKET_MAX) {
-        k_fold_slice_warp<<<(unsigned)((n_act + GD_LP_WARPS - 1) / GD_LP_WARPS), GD_LP_THREADS, 0, c->stream>>>(c->d, c->slice_grid, sa);
+        k_fold_slice_warp<<<(unsigned)((n_act + GD_LP_WARPS - 1) / GD_LP_WARPS), GD_LP_THREADS, 0, c->stream>>>(c->d, c->slice_grid * c->slice_passes, sa);
         GD_LAUNCH_CHECK(c, "k_fold_slice_warp");
     }
     return 0;

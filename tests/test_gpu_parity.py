@@ -79,16 +79,19 @@ KERNEL_OPTIONS = {   # force one of the four force kernels regardless of n_act
     "ipar_small": {"slice_max_nact": 0, "jsplit_max_nact": 0, "ipar_small_max_nact": 1 << 30},
     "jsplit": {"slice_max_nact": 0, "jsplit_max_nact": 1 << 30},   # capped by the library at 32 sinks x the clusters of its grid
     "slice": {"slice_max_nact": 1 << 30},
+    "slice3": {"slice_max_nact": 1 << 30, "slice_passes": 3},     # three slices per CTA, as for systems beyond shared memory
 }
 
 
-@pytest.mark.parametrize("kernel", ["ipar", "ipar_small", "jsplit", "slice"])
+@pytest.mark.parametrize("kernel", ["ipar", "ipar_small", "jsplit", "slice", "slice3"])
 @pytest.mark.parametrize("n_act", [1, 5, 16, 96, 97, 100, 256, 1000, 4096])
 def test_force_active_subsets_all_kernels(gd, kernel, n_act):
     # C3-style index sets on a smaller sphere, forced through each kernel; all must agree with the oracle
     import torch
     if kernel == "jsplit" and n_act > 1000:
         pytest.skip("beyond the j-split kernel's grid (32 sinks per cluster)")
+    if kernel == "slice3" and n_act > 2048:
+        pytest.skip("beyond the partial-sum scratch of three slices per CTA at this N")
     w = W.config(3, n=8192 + 77)
     h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
     for key, val in KERNEL_OPTIONS[kernel].items():
@@ -96,7 +99,9 @@ def test_force_active_subsets_all_kernels(gd, kernel, n_act):
     h.predict(0.0)
     idx = W.active_indices(w.n, n_act)
     a, j = h.force_jerk(torch.from_numpy(idx).cuda())
-    assert h.last_force_kernel == kernel
+    assert h.last_force_kernel == kernel.rstrip("3")
+    if kernel.startswith("slice"):
+        assert h.last_force_geometry[3] == (3 if kernel == "slice3" else 1)
     a_ref, j_ref = oracle.pairsum(w.m, w.x, w.v, w.eps, idx=idx)
     assert relnorm(cpu(a), a_ref).max() <= TOL and relnorm(cpu(j), j_ref).max() <= TOL
     # run-to-run identical (fixed combination order)
@@ -307,8 +312,9 @@ def test_host_init_equals_device_init(gd):
 
 
 # ------------------------------------------------------------------------------ the captured block-step graph
+@pytest.mark.parametrize("slice_on", [True, False])
 @pytest.mark.parametrize("cfg,n", [(1, 1024), (4, 3000), (5, 2047)])
-def test_graph_replay_equals_explicit_calls(gd, cfg, n):
+def test_graph_replay_equals_explicit_calls(gd, cfg, n, slice_on):
     # gd_run_until / gd_step replay a captured graph whose kernels read n_act and t_next from device memory;
     # the explicit call sequence passes them from the host.  Same kernels, same arithmetic: identical bits.
     w = W.config(cfg, n=n)
@@ -316,7 +322,12 @@ def test_graph_replay_equals_explicit_calls(gd, cfg, n):
     he = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
     hg.set_option("loop_max_nact", 0)            # stage kernels only: the persistent loop sums in another order
     he.set_option("use_graph", 0)
-    he.set_option("slice_max_nact", 0)           # ... and so does k_force_slice, which the graph does not hold
+    if slice_on:
+        for u in (hg, he):
+            u.set_option("slice_passes", 3)      # k_force_slice with three slices per CTA, as at C5's size
+    else:
+        for u in (hg, he):
+            u.set_option("slice_max_nact", 0)    # k_force_jsplit / k_force_ipar take every step
     for steps in (40, 70):                       # 70 is not a multiple of the graph's step count
         pg = hg.step(steps)
         pe = he.step(steps)
