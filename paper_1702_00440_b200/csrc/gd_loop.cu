@@ -943,6 +943,21 @@ k_fold_slice_warp(gd_dev d, int G, gd_sargs sa)
 // Geometry: one CTA per SM; S = slice capacity (multiple of 32); hi = largest active set taken, bounded by the option
 // `loop_max_nact` and by the partial-sum scratch (grid x 6 x cap doubles).  loop_grid = 0: the loop is not usable
 // (slice does not fit in shared memory, or the device cannot co-schedule the grid) and the stage kernels run alone.
+// dynamic shared memory a kernel may use: the device's opt-in maximum minus the kernel's static shared memory.  The limit
+// is a property of the function, not of a context, so it is raised to that maximum once for every instantiation:
+// contexts of different sizes can then coexist.
+template <typename K>
+static int gd_raise_smem_limit(gd_ctx *c, K kernel, int max_optin, size_t *avail)
+{
+    cudaFuncAttributes fa;
+    GD_CUDA(c, cudaFuncGetAttributes(&fa, kernel));
+    const int lim = max_optin - (int)fa.sharedSizeBytes;
+    if (lim <= 0) { *avail = 0; return 0; }
+    GD_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+    if ((size_t)lim < *avail) *avail = (size_t)lim;
+    return 0;
+}
+
 int gdk_loop_setup(gd_ctx *c)
 {
     c->loop_grid = 0;
@@ -958,12 +973,13 @@ int gdk_loop_setup(gd_ctx *c)
     GD_CUDA(c, cudaGetDevice(&dev));
     GD_CUDA(c, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     GD_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    size_t avail = (size_t)max_smem;
+    if (gd_raise_smem_limit(c, k_block_loop<false>, max_smem, &avail) || gd_raise_smem_limit(c, k_block_loop<true>, max_smem, &avail))
+        return -3;                                           // GD_ECUDA; text already in c->err
     int state = c->loop_state_opt ? 1 : 0;
     size_t bytes = gd_lsm_bytes((int)S, state);
-    if (bytes > (size_t)max_smem) { state = 0; bytes = gd_lsm_bytes((int)S, 0); }
-    if (!coop || bytes > (size_t)max_smem) return 0;
-    GD_CUDA(c, cudaFuncSetAttribute(k_block_loop<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-    GD_CUDA(c, cudaFuncSetAttribute(k_block_loop<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    if (bytes > avail) { state = 0; bytes = gd_lsm_bytes((int)S, 0); }
+    if (!coop || bytes > avail) return 0;
     int resident = 0;
     GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_block_loop<false>, GD_LP_THREADS, bytes));
     if (resident < 1) return 0;
@@ -1015,6 +1031,9 @@ int gdk_slice_setup(gd_ctx *c)
     GD_CUDA(c, cudaGetDevice(&dev));
     GD_CUDA(c, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     // passes: the fewest slices per CTA whose records fit in shared memory (option `slice_passes` forces a count)
+    size_t avail = (size_t)max_smem;
+    if (gd_raise_smem_limit(c, k_force_slice<false>, max_smem, &avail) || gd_raise_smem_limit(c, k_force_slice<true>, max_smem, &avail))
+        return -3;                                           // GD_ECUDA; text already in c->err
     int64_t S = 0;
     size_t bytes = 0;
     int passes = c->slice_passes_opt > 0 ? (int)c->slice_passes_opt : 1;
@@ -1022,11 +1041,9 @@ int gdk_slice_setup(gd_ctx *c)
         S = (c->n + (int64_t)grid * passes - 1) / ((int64_t)grid * passes);
         S = (S + 31) / 32 * 32;
         bytes = gd_lsm_bytes((int)S, 0);
-        if (bytes <= (size_t)max_smem) break;
+        if (bytes <= avail) break;
         if (c->slice_passes_opt > 0 || passes >= GD_SL_MAX_PASSES) return 0;
     }
-    GD_CUDA(c, cudaFuncSetAttribute(k_force_slice<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-    GD_CUDA(c, cudaFuncSetAttribute(k_force_slice<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     c->slice_grid = grid;
     c->slice_passes = passes;
     c->slice_S = (int)S;
