@@ -109,3 +109,28 @@ def test_two_body_closed_form_setup():
     vrel = np.linalg.norm(w.v[1] - w.v[0])
     assert abs(vrel - 1.0) < 1e-14               # circular: v^2 = M/r
     assert np.abs((w.m[:, None] * w.v).sum(0)).max() < 1e-16
+
+
+@pytest.mark.parametrize("cfg,n", [(3, 65536), (4, 262144), (5, 1048577)])
+def test_stored_full_size_schedules_are_well_formed(cfg, n):
+    # tests/golden/c<k>_full_schedule.txt (the oracle's first 100 block steps at full size, written by
+    # tests/golden/make_full_size_schedule.py): times strictly increasing dyadic values, counts consistent with the
+    # totals, the level histogram sums to the particle steps, 64 samples inside the system
+    from conftest import GOLDEN
+    steps, kv, samples = [], {}, []
+    for line in (GOLDEN / f"c{cfg}_full_schedule.txt").read_text().splitlines():
+        tok = line.split("#", 1)[0].split()
+        if not tok:
+            continue
+        if tok[0] == "step":
+            steps.append((float.fromhex(tok[1]), int(tok[2])))
+        elif tok[0] == "sample":
+            samples.append(int(tok[1]))
+        else:
+            kv[tok[0]] = tok[1:]
+    assert len(steps) == 100 and len(samples) == 64 and all(0 <= i < n for i in samples)
+    t = np.array([s[0] for s in steps])
+    assert np.all(np.diff(t) > 0) and np.all(t * 2.0 ** 23 == np.round(t * 2.0 ** 23))
+    assert all(1 <= s[1] <= n for s in steps)
+    assert sum(s[1] for s in steps) == int(kv["particle_steps"][0]) == sum(int(c) for c in kv["level_hist"])
+    assert float(kv["min_margin"][0]) > 1e-10 and int(kv["nan_count"][0]) == 0
