@@ -29,7 +29,9 @@
 #include "gd_pair.cuh"
 #include <limits.h>
 
-#define GD_LP_THREADS 256
+#ifndef GD_LP_THREADS
+#define GD_LP_THREADS 256          // threads of the one CTA per SM (a multiple of 32; tuning knob)
+#endif
 #define GD_LP_WARPS (GD_LP_THREADS / 32)
 #define GD_LP_MAX_GRID 256          // CTAs (one per SM); bounds the shared tables
 #define GD_LP_MAX_SMALL 256         // largest active set of the lanes-over-sources mapping (bounds the position map)
@@ -203,7 +205,7 @@ __device__ __forceinline__ int gd_publish(const gd_dev &d, const gd_lsm &sm, int
     m = gd_warp_min_d(m);
     if (lane == 0) sm.wmin[warp] = m;
     __syncthreads();
-    m = sm.wmin[lane & (GD_LP_WARPS - 1)];
+    m = lane < GD_LP_WARPS ? sm.wmin[lane] : GD_INF;
     m = gd_warp_min_d(m);
     const double L = m;
     int base = 0;
@@ -488,7 +490,7 @@ __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &s
     // enough to be split over the warps of a tile (measured: N = 65536, 256 sinks: 44 us against 76 us with narrow
     // tiles; N = 16384 the other way round).
     if (n_act >= 2 * 64 * GD_LP_WARPS || cnt_own >= 256) {
-        if (gd_lp_balance((n_act + 127) >> 7) + 5 >= gd_lp_balance((n_act + 63) >> 6))
+        if (GD_LP_THREADS <= 256 && gd_lp_balance((n_act + 127) >> 7) + 5 >= gd_lp_balance((n_act + 63) >> 6))
             gd_lp_force_wide<4, EPS0>(d, sm, la, out, rs, G, n_act, cnt_own);
         else
             gd_lp_force_wide<2, EPS0>(d, sm, la, out, rs, G, n_act, cnt_own);
@@ -695,7 +697,7 @@ k_block_loop(gd_dev d, gd_largs la)
         double m = gd_warp_min_d(Lc);
         if (lane == 0) sm.wmin[warp] = m;
         __syncthreads();
-        m = gd_warp_min_d(sm.wmin[lane & (GD_LP_WARPS - 1)]);
+        m = gd_warp_min_d(lane < GD_LP_WARPS ? sm.wmin[lane] : GD_INF);
         const double t_next = m;
         const int mine = (tid < G && Lc == t_next) ? cc : 0;
         int incl = mine;
@@ -716,7 +718,7 @@ k_block_loop(gd_dev d, gd_largs la)
             for (int k = 0; k < mine; ++k) sm.smap[excl + k] = r0 + k;
         }
         // small mode: the sink records are fetched (L2) while the own slice is predicted
-        constexpr int NPF = GD_LP_MAX_SMALL * 4 / GD_LP_THREADS;
+        constexpr int NPF = (GD_LP_MAX_SMALL * 4 + GD_LP_THREADS - 1) / GD_LP_THREADS;
         double2 pf[NPF];
         if (small) {
             __syncthreads();                                 // smap is complete
