@@ -347,9 +347,9 @@ def main_ours(args):
 
 
 # dram bytes per launch of the dominant force kernel from the committed `ncu --set full` capture under profiles/
-# (None until one exists for the workload; see profiles/README.md)
+# (None until one exists for the workload)
 NCU_TRAFFIC_BYTES = {("C2", "jsplit"): 938240, ("C2", "ipar"): 934656, ("C2", "ipar_small"): 936192,   # profiles/r1c_launches_graph_path.md
-                     ("C2", "loop"): 14855294000}                                                # profiles/r1h_final_round1.md
+                     ("C2", "loop"): 14877042000}                                                # profiles/r1r_final_round1.md
 KERNEL_NAMES = {"ipar": "k_force_ipar<2,1>", "jsplit": "k_force_jsplit", "ipar_small": "k_force_ipar<1,4>",
                 "loop": "k_block_loop", "slice": "k_force_slice"}
 
