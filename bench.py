@@ -211,8 +211,8 @@ def stage_bandwidth(gd, torch, W):
 
     rows = {}
     # the usual case first: the first block of C5 under its own block steps (a handful of active particles)
-    h.next_block()
-    s_nb, (_, n_first) = timed(h.next_block, 5)
+    _, n_first = h.next_block()
+    s_nb = statistics.median(timed(h.next_block)[0] for _ in range(9))     # median of nine single calls
     rows["next_block"] = {"us": round(s_nb * 1e6, 2), "n_act": n_first, "algorithmic_bytes": 16.0 * w.n + 4.0 * n_first,
                           "gbs": (16.0 * w.n + 4.0 * n_first) / s_nb / 1e9, "frac_hbm": (16.0 * w.n + 4.0 * n_first) / s_nb / 1e9 / peak,
                           "note": "per call, including the device-to-host copy of (t_next, n_act) and the stream synchronisation"}
