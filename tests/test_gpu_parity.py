@@ -517,3 +517,56 @@ def test_lagrange_radii_follow_the_predicted_state_and_reject_bad_fractions(gd):
         with pytest.raises(gd.GravidyError):
             h.lagrange_radii(bad)
     h.close()
+
+
+# ------------------------------------------------------------------------------ options that change the schedule
+@pytest.mark.parametrize("use_loop", [True, False])
+def test_single_halving_variant_matches_oracle(gd, use_loop):
+    # DESIGN.md reading R7: the block rule's variant "a single halving per step" (halving_mode 0) on both sides
+    w = W.config(4, n=1500)                      # the variants part ways at block step 53 of this input
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h.set_option("halving_mode", 0)
+    if not use_loop:
+        h.set_option("loop_max_nact", 0)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta, halving_mode=0)
+    psteps = h.step(150)
+    for _ in range(150):
+        o.step()
+    s = h.state_host(("x", "t", "dt"))
+    assert h.t == o.t and psteps == o.particle_steps
+    assert np.array_equal(s["t"], o.t_i) and np.array_equal(s["dt"], o.dt) and np.abs(s["x"] - o.x).max() < 1e-12
+    # the two variants do differ on this input (otherwise the test would not tell them apart)
+    o1 = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta, halving_mode=1)
+    for _ in range(150):
+        o1.step()
+    assert o1.particle_steps != o.particle_steps or not np.array_equal(o1.dt, o.dt)
+    h.close()
+
+
+@pytest.mark.parametrize("level", [6, 9])
+def test_shared_step_special_case_matches_oracle(gd, level):
+    # SURVEY 8(c) pin 7: dt_min = dt_max makes the scheme the shared-step 4th-order Hermite integrator; every particle
+    # is active in every step.  Device: options dt_level_min = dt_level_max; oracle: dt_min = dt_max = 2^-level.
+    w = W.config(4, n=1500)
+    dt = 2.0 ** -level
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h.set_option("dt_level_min", level)
+    h.set_option("dt_level_max", level)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta, dt_min=dt, dt_max=dt)
+    for k in range(12):
+        t_next, n_act = h.next_block()
+        assert n_act == w.n and t_next == (k + 1) * dt
+        h.predict(t_next)
+        h.force_jerk(None)
+        h.correct_and_timestep()
+        o.step()
+    s = h.state_host()
+    assert np.array_equal(s["t"], o.t_i) and np.array_equal(s["dt"], o.dt)
+    assert np.abs(s["x"] - o.x).max() < 1e-12 and np.abs(s["v"] - o.v).max() < 1e-12
+    assert relnorm(s["a"], o.a).max() < 1e-11 and relnorm(s["j"], o.j).max() < 1e-11
+    k1, u1 = h.energy()
+    k2, u2 = o.energy()
+    assert abs((k1 + u1) / (k2 + u2) - 1.0) < 1e-11
+    with pytest.raises(gd.GravidyError):
+        h.set_option("dt_level_max", level + 1)          # levels can only change before the first step
+    h.close()
