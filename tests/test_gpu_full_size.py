@@ -171,3 +171,24 @@ def test_c5_workload_all_active_plus_10_block_steps_invariants(gd):
     k1, u1 = h.energy()
     assert abs((k1 + u1) / (k0 + u0) - 1.0) < 1e-9      # 10 tiny block steps: the energy has not moved
     h.close()
+
+
+def test_contexts_of_different_sizes_coexist(gd):
+    # the dynamic shared-memory limit is a property of the kernel function, not of a context: a small context created
+    # after a large one must not shrink what the large one may launch with (k_force_slice: 160 KB of source records
+    # per CTA at N = 200000; k_block_loop likewise)
+    import torch
+    big = W.config(4, n=200000)
+    small = W.config(1)
+    hb = gd.Hermite(big.m, big.x, big.v, big.eps, big.eta)
+    hs = gd.Hermite(small.m, small.x, small.v, small.eps, small.eta)
+    hb.predict(0.0)
+    idx = W.active_indices(big.n, 100, seed=11)
+    a, j = hb.force_jerk(torch.from_numpy(idx).cuda())
+    assert hb.last_force_kernel == "slice"
+    a_ref, j_ref = oracle.pairsum(big.m, big.x, big.v, big.eps, idx=idx)
+    assert relnorm(cpu(a), a_ref).max() <= TOL and relnorm(cpu(j), j_ref).max() <= TOL
+    assert hb.step(40) > 0 and hs.step(40) > 0 and hb.step(40) > 0       # both persistent loops, interleaved
+    assert hb.loop_profile()["block_steps"] == 80 and hs.loop_profile()["block_steps"] == 40
+    check_invariants(hb.state_host(("t", "dt")), hb.t)
+    hb.close(); hs.close()
