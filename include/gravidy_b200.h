@@ -180,6 +180,11 @@ GD_API int gd_lagrange_radii(gd_ctx *ctx, const double *center_host, const doubl
  * corrector phase, in the barrier after it, launches that did work, and for CTA 0 as an owner of active particles:
  * steps, ns summing partials + correcting, ns publishing } (11 values).  Synchronises. */
 GD_API int gd_get_loop_profile(gd_ctx *ctx, int64_t *out_host);
+/* The same loop's block steps binned by the size of their active set ("N_act << N": where the step count and the
+ * time of a block-step run go) -> out_host[32][6]: bucket b holds the steps with bit_length(n_act) == b, i.e.
+ * 2^(b-1) <= n_act < 2^b, as { block steps, particle steps, ns in the force phase, ns in the barrier after it, ns in
+ * the corrector phase, ns in the barrier after it } (device global timer, CTA 0's view), since init.  Synchronises. */
+GD_API int gd_get_loop_histogram(gd_ctx *ctx, int64_t *out_host);
 
 /* Optional CUDA-event timing of the force launches, switched on with gd_set_option(ctx, "profile", 1): every
  * gd_force_jerk issued afterwards is bracketed by two events on the context's stream (the all-active evaluation

@@ -51,6 +51,7 @@ SYMBOLS = {
     "gd_get_level_histogram": (_int, [_vp, _vp, _vp]),
     "gd_get_profile": (_int, [_vp, _vp]),
     "gd_get_loop_profile": (_int, [_vp, _vp]),
+    "gd_get_loop_histogram": (_int, [_vp, _vp]),
     "gd_lagrange_radii": (_int, [_vp, _vp, _vp, _int, _vp, _vp]),
     "gd_fp64_peak_probe": (_int, [_int, _pdbl, _pdbl]),
     "gd_selftest_div_const": (_int, [C.c_int64, C.c_uint64, _vp]),
@@ -329,6 +330,13 @@ class Hermite:
         keys = ("particle_steps", "block_steps", "ns", "ns_force", "ns_barrier1", "ns_correct", "ns_barrier2", "launches",
                 "owner_steps", "ns_owner_correct", "ns_owner_publish")
         return {k: int(v) for k, v in zip(keys, o)}
+
+    def loop_histogram(self) -> list[dict]:
+        """Block steps of the persistent loop binned by active-set size: one row per non-empty bucket."""
+        o = np.zeros((32, 6), dtype=np.int64)
+        self._check(self._lib.gd_get_loop_histogram(self._h, o.ctypes.data))
+        keys = ("block_steps", "particle_steps", "ns_force", "ns_barrier1", "ns_correct", "ns_barrier2")
+        return [dict({"n_act_below": 1 << b}, **{k: int(v) for k, v in zip(keys, o[b])}) for b in range(32) if o[b, 0]]
 
     def level_histogram(self) -> tuple[np.ndarray, np.ndarray]:
         h, d = np.zeros(64, dtype=np.int64), np.zeros(2, dtype=np.int64)

@@ -118,6 +118,7 @@ static size_t gd_carve(gd_dev *d, void *base, int64_t np, int64_t pcap)
     t.lp_L = w.take<double>(256);
     t.lp_cnt = w.take<int>(256);
     t.lp_ctl = w.take<unsigned long long>(16);
+    t.lp_prof = w.take<unsigned long long>(GD_LP_PROF_BUCKETS * 6);
     t.diag_scratch = w.take<unsigned long long>(4352);
     t.cell = w.take<double>(4);
     t.hist = w.take<long long>(64);
@@ -644,6 +645,23 @@ extern "C" int gd_get_loop_profile(gd_ctx *c, int64_t *out_host)
 {
     if (!c || !out_host) return GD_EINVAL;
     GD_CUDA(c, cudaMemcpyAsync(out_host, c->d.lp_ctl + 2, 11 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return GD_OK;
+}
+
+#if GD_LP_FINE
+extern "C" __attribute__((visibility("default"))) int gd_debug_read_staging(gd_ctx *c, void *host, size_t nbytes)
+{
+    GD_CUDA(c, cudaMemcpyAsync(host, c->d.staging, nbytes, cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return GD_OK;
+}
+#endif
+
+extern "C" int gd_get_loop_histogram(gd_ctx *c, int64_t *out_host)
+{
+    if (!c || !out_host) return GD_EINVAL;
+    GD_CUDA(c, cudaMemcpyAsync(out_host, c->d.lp_prof, GD_LP_PROF_BUCKETS * 6 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
     GD_CUDA(c, cudaStreamSynchronize(c->stream));
     return GD_OK;
 }

@@ -53,7 +53,13 @@ struct gd_dev {
     int *lp_cnt;                 // [256] candidates per CTA
     unsigned long long *lp_ctl;  // [16] {barrier arrivals, arrivals at the start of the current launch, then profiling counters:
                                  //  particle steps, block steps, ns in the loop, ns per phase x 4, launches that ran}
+    unsigned long long *lp_prof; // [GD_LP_PROF_BUCKETS][6] per bucket b = bit length of n_act: {block steps, particle steps,
+                                 //  ns in [force], in the barrier after it, in [correct], in the barrier after it} (CTA 0's view)
 };
+#define GD_LP_PROF_BUCKETS 32
+#ifndef GD_LP_FINE
+#define GD_LP_FINE 0               // 1: debug build with fine-grained phase stamps of the loop (gd_loop.cu)
+#endif
 
 #define GD_SCAN_MAX_BLOCKS 1024
 #define GD_LP_REC_SLACK (32 * 256)   // rows of lp_rec beyond np: slices are rounded up to 32 for up to 256 CTAs

@@ -33,6 +33,9 @@
 #define GD_LP_THREADS 256          // threads of the one CTA per SM (a multiple of 32; tuning knob)
 #endif
 #define GD_LP_WARPS (GD_LP_THREADS / 32)
+#ifndef GD_LP_PROFILE
+#define GD_LP_PROFILE 1            // 0: no device-timer reads inside the loop (gd_get_loop_profile / _histogram then report 0 ns)
+#endif
 #ifndef GD_LP_ITEM_UNROLL
 #define GD_LP_ITEM_UNROLL 2        // unrolling of the round loop of a lanes-over-sources item
 #endif
@@ -88,7 +91,9 @@ __device__ __forceinline__ void gd_bar_wait(unsigned long long *bar, unsigned lo
 __device__ __forceinline__ unsigned long long gd_gtime()
 {
     unsigned long long t = 0;
+#if GD_LP_PROFILE
     if (blockIdx.x == 0 && threadIdx.x == 0) asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+#endif
     return t;
 }
 
@@ -541,6 +546,17 @@ __device__ __forceinline__ void gd_lp_force_big(const gd_dev &d, const gd_lsm &s
 }
 
 
+// fine-grained phase stamps of a debug build (-DGD_LP_FINE=1): per CTA, thread 0's clock64 deltas of the steps with
+// n_act <= GD_LP_FINE_MAX, summed into d.staging as [CTA][16] {cycles x 12, -, -, steps, owner steps}
+#ifndef GD_LP_FINE_MAX
+#define GD_LP_FINE_MAX 8
+#endif
+#if GD_LP_FINE
+#define GD_STAMP(k) do { if (tid == 0) { const long long c_ = clock64(); if (fine_on) fine[k] += c_ - fine_last; fine_last = c_; } } while (0)
+#else
+#define GD_STAMP(k) do { } while (0)
+#endif
+
 // ---- [correct] -----------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void gd_lp_commit(const gd_dev &d, const gd_lsm &sm, int i, int p, double m, const gd_corrected &r,
                                              const double (&a1)[3], const double (&j1)[3], double h, double t_next)
@@ -696,6 +712,10 @@ k_block_loop(gd_dev d, gd_largs la)
     bool fin = false;
     unsigned long long tr[4] = {0, 0, 0, 0}, own[3] = {0, 0, 0}, g0 = gd_gtime(), g1;   // CTA 0's view: ns in [force], barrier, [correct], barrier
     const unsigned long long g_begin = g0;
+#if GD_LP_FINE
+    long long fine[16] = {0}, fine_last = clock64();
+    bool fine_on = false;
+#endif
     for (;;) {
         if (t_cur >= t_end || (max_steps >= 0 && steps >= max_steps)) { fin = true; break; }
         // ---- [force] ----
@@ -707,6 +727,7 @@ k_block_loop(gd_dev d, gd_largs la)
         __syncthreads();
         m = gd_warp_min_d(lane < GD_LP_WARPS ? sm.wmin[lane] : GD_INF);
         const double t_next = m;
+        GD_STAMP(0);
         const int mine = (tid < G && Lc == t_next) ? cc : 0;
         int incl = mine;
 #pragma unroll
@@ -717,6 +738,9 @@ k_block_loop(gd_dev d, gd_largs la)
 #pragma unroll
         for (int w = 0; w < GD_LP_WARPS; ++w) { int c = sm.wcnt[w]; wbase += (w < warp) ? c : 0; n_act += c; }
         if (n_act > la.hi) break;                            // uniform: the stage kernels take this step
+#if GD_LP_FINE
+        fine_on = n_act <= GD_LP_FINE_MAX;
+#endif
         const bool small = n_act <= la.small_hi;
         const int excl = wbase + incl - mine;
         if (tid < G) sm.spre[tid] = excl;
@@ -736,6 +760,7 @@ k_block_loop(gd_dev d, gd_largs la)
                 if (e < 4 * n_act) pf[u] = __ldcg(reinterpret_cast<const double2 *>(d.lp_rec) + 4 * (size_t)sm.smap[e >> 2] + (e & 3));
             }
         }
+        GD_STAMP(1);
         // own slice predicted to t+
         for (int p = tid; p < cnt_own; p += GD_LP_THREADS) {
             const int i = p0 + p;
@@ -754,13 +779,17 @@ k_block_loop(gd_dev d, gd_largs la)
             }
         }
         __syncthreads();
+        GD_STAMP(2);
         if (small) gd_lp_force_small<EPS0>(d, sm, la, out, rs, n_act, rounds);
         else gd_lp_force_big<EPS0>(d, sm, la, out, rs, G, n_act, cnt_own);
-        g1 = gd_gtime(); tr[0] += g1 - g0; g0 = g1;
+        GD_STAMP(3);
+        g1 = gd_gtime(); const unsigned long long d0 = g1 - g0; tr[0] += d0; g0 = g1;
         gd_bar_arrive(bar);
+        GD_STAMP(4);
         target += G;
         gd_bar_wait(bar, target);
-        g1 = gd_gtime(); tr[1] += g1 - g0; g0 = g1;
+        GD_STAMP(5);
+        g1 = gd_gtime(); const unsigned long long d1 = g1 - g0; tr[1] += d1; g0 = g1;
         // ---- [correct] + [publish] ----
         const bool contributing = (L_me == t_next) && cnt_me > 0;
         if (contributing) {
@@ -773,20 +802,41 @@ k_block_loop(gd_dev d, gd_largs la)
                 for (int k = tid; k < cnt_me; k += GD_LP_THREADS) gd_lp_correct_thread(d, sm, la, G, p0, pre + k, sm.lact[k], t_next);
             }
             __syncthreads();
+            GD_STAMP(6);
             const unsigned long long o1 = gd_gtime();
             cnt_me = gd_publish(d, sm, me, p0, cnt_own, &L_me);
+            GD_STAMP(7);
+#if GD_LP_FINE
+            if (tid == 0 && fine_on) fine[15] += 1;
+#endif
             own[0] += 1; own[1] += o1 - o0; own[2] += gd_gtime() - o1;
         }
         t_cur = t_next;
         steps += 1;
         psteps += n_act;
-        g1 = gd_gtime(); tr[2] += g1 - g0; g0 = g1;
+        g1 = gd_gtime(); const unsigned long long d2 = g1 - g0; tr[2] += d2; g0 = g1;
+        GD_STAMP(8);
         gd_bar_arrive(bar);
+        GD_STAMP(9);
         target += G;
         gd_bar_wait(bar, target);
-        g1 = gd_gtime(); tr[3] += g1 - g0; g0 = g1;
+        GD_STAMP(10);
+#if GD_LP_FINE
+        if (tid == 0 && fine_on) fine[14] += 1;
+#endif
+        g1 = gd_gtime(); const unsigned long long d3 = g1 - g0; tr[3] += d3; g0 = g1;
+#if GD_LP_PROFILE
+        if (me == 0 && tid == 0) {                           // per-size bins of gd_get_loop_histogram (fire-and-forget REDs)
+            unsigned long long *hb = d.lp_prof + 6 * (32 - __clz(n_act));
+            atomicAdd(hb, 1ull); atomicAdd(hb + 1, (unsigned long long)n_act);
+            atomicAdd(hb + 2, d0); atomicAdd(hb + 3, d1); atomicAdd(hb + 4, d2); atomicAdd(hb + 5, d3);
+        }
+#endif
     }
 
+#if GD_LP_FINE
+    if (tid == 0) for (int k = 0; k < 16; ++k) ((long long *)d.staging)[me * 16 + k] = fine[k];
+#endif
     // ---- leave: flush the counters; CTA 0 hands the run state back ----
     if (tid < 64 && sm.hist[tid]) atomicAdd((unsigned long long *)&d.hist[tid], (unsigned long long)sm.hist[tid]);
     if (tid < 2 && sm.hist[64 + tid]) atomicAdd((unsigned long long *)&d.diag[tid], (unsigned long long)sm.hist[64 + tid]);
