@@ -111,7 +111,11 @@ __device__ __forceinline__ double gd_new_step(double na1, double nj1, double na2
         if (halving_mode == 1)
             while (dnew > dt_req && dnew > dt_min) dnew *= 0.5;
     } else if (dt_req >= 2.0 * h) {
-        double q = t_next / (2.0 * h);                        // exact: 2h is a power of two
+        // t_next / 2h: exact when 2h is a power of two (always, for block steps), and then the same double as the product
+        // with the exactly representable 1 / 2h -- one multiplication instead of the division routine
+        const long long hb = __double_as_longlong(h), ef = (hb >> 52) & 0x7ff;
+        const bool pow2 = hb > 0 && (hb & 0xfffffffffffffLL) == 0 && ef >= 1023 - 300 && ef <= 1023 + 300;
+        const double q = pow2 ? t_next * __longlong_as_double((2045LL - ef) << 52) : t_next / (2.0 * h);
         if (q == floor(q)) dnew = 2.0 * h;
     }
     if (dnew < dt_min) dnew = dt_min;

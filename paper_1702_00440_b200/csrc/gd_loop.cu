@@ -269,7 +269,7 @@ __device__ __forceinline__ gd_src gd_lp_load_sink(const gd_dev &d, int row_index
 // ---- [force], small mode: lanes stride over the own sources ------------------------------------------------------------
 // BI sinks (active-list positions pos0 .. pos0 + BI - 1) against the source rounds [r_begin, r_end) of the own
 // slice; lane l takes source 32 r + l.  Returns the 6 BI per-lane sums in v[b * 6 + {ax, ay, az, jx, jy, jz}].
-template <int BI, bool EPS0>
+template <int BI, bool EPS0, int UNR = GD_LP_ITEM_UNROLL>
 __device__ __forceinline__ void gd_lp_item(const gd_dev &d, const gd_lsm &sm, int pos0, int r_begin, int r_end, int lane,
                                            double eps2, double *v)
 {
@@ -282,7 +282,7 @@ __device__ __forceinline__ void gd_lp_item(const gd_dev &d, const gd_lsm &sm, in
         si[b] = gd_src{xy.x, xy.y, zi.x, 0.0, wxy.x, wxy.y, wz.x};
         acc[b] = gd_acc{0, 0, 0, 0, 0, 0};
     }
-    GD_LP_PRAGMA_UNROLL(GD_LP_ITEM_UNROLL)
+    GD_LP_PRAGMA_UNROLL(UNR)
     for (int r = r_begin; r < r_end; ++r) {
         const int j = r * 32 + lane;
         const double2 xy = sm.pxy[j], zm = sm.pzm[j], vxy = sm.vxy[j];
@@ -314,6 +314,16 @@ template <bool EPS0>
 __device__ __forceinline__ void gd_lp_force_small(const gd_dev &d, const gd_lsm &sm, const gd_largs &la, double *out, int rs, int n_act, int rounds)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (n_act <= GD_LP_WARPS && rounds <= 8) {               // a handful of sinks against a short slice: a warp per sink, no hand-off
+        if (warp < n_act) {
+            double v[6];
+            gd_lp_item<1, EPS0, 4>(d, sm, warp, 0, rounds, lane, la.eps2, v);
+            gd_rs6(v, lane);
+            const int e = gd_rs6_elem(lane);
+            if (e >= 0) gd_lp_put(out, rs, warp, e, v[0]);
+        }
+        return;
+    }
     const int n4 = n_act >> 2, items = n4 + (n_act & 3);
     if (items >= GD_LP_WARPS) {
         for (int it = warp; it < items; it += GD_LP_WARPS) {
@@ -340,7 +350,7 @@ __device__ __forceinline__ void gd_lp_force_small(const gd_dev &d, const gd_lsm 
     const bool four = it < n4;
     const int pos = four ? 4 * it : 4 * n4 + (it - n4);
     if (work) {
-        const int rb = (int)((long long)rounds * chunk / nsplit), re = (int)((long long)rounds * (chunk + 1) / nsplit);
+        const int rb = rounds * chunk / nsplit, re = rounds * (chunk + 1) / nsplit;
         if (four) {
             double v[24];
             gd_lp_item<4, EPS0>(d, sm, pos, rb, re, lane, la.eps2, v);
@@ -689,6 +699,7 @@ k_block_loop(gd_dev d, gd_largs la)
     unsigned long long target = d.lp_ctl[1];
     double *out = d.partial + (size_t)me * 6;
     const int rs = 6 * G;
+    const int r0_tid = gd_slice_begin(tid < G ? tid : 0, la.n, G);   // first row of the segment of CTA `tid` (a 64-bit division: once)
 
     for (int p = tid; p < rounds * 32; p += GD_LP_THREADS) {
         if (p < cnt_own) {
@@ -746,8 +757,7 @@ k_block_loop(gd_dev d, gd_largs la)
         if (tid < G) sm.spre[tid] = excl;
         if (tid == 0) sm.spre[G] = n_act;
         if (small && mine > 0) {
-            const int r0 = gd_slice_begin(tid, la.n, G);
-            for (int k = 0; k < mine; ++k) sm.smap[excl + k] = r0 + k;
+            for (int k = 0; k < mine; ++k) sm.smap[excl + k] = r0_tid + k;
         }
         // small mode: the sink records are fetched (L2) while the own slice is predicted
         constexpr int NPF = (GD_LP_MAX_SMALL * 4 + GD_LP_THREADS - 1) / GD_LP_THREADS;
