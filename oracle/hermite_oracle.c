@@ -19,8 +19,10 @@
  *
  * Pins (tests/test_oracle_*.py): Kepler closed form, momentum invariants, jerk finite difference,
  * long-double brute force, mpmath brute force, exact-polynomial corrector test, 4th-order
- * convergence, Plummer energy drift, Listing-1 statistics, scheduler invariants.
- * Parity unpinned (paper silent): initial-dt rule, dt_min, the block up/down rule.
+ * convergence, Plummer energy drift, Listing-1 statistics, scheduler invariants, hand numbers for the
+ * initial step (orc_initial_dt), and for the block rule the paper's energy accuracy at eta = 0.01
+ * on the stored C2 runs under both readings (tests/golden/c2_t1_energy*.txt).
+ * Parity unpinned (paper silent): the value of dt_min (2^-23) only.
  */
 #include <math.h>
 #include <stdint.h>

@@ -1,7 +1,7 @@
 """ctypes wrapper around oracle/hermite_oracle.c -- TEST INFRASTRUCTURE, not product.
 
 Argument marshalling only; every formula lives in the C file, which cites the paper passage it follows.
-Parity unpinned (paper silent): initial-dt rule, dt_min, block up/down rule.
+Parity unpinned (paper silent): the value of dt_min only.
 """
 from __future__ import annotations
 

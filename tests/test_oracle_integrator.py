@@ -111,6 +111,43 @@ def test_block_init():
         assert d <= val < 2 * d and math.log2(d) == round(math.log2(d))
 
 
+def test_initial_dt_hand_numbers():
+    # INIT, step (iv) ("from the initial calculation"; reading R4): dt = eta |a| / |jerk| with Euclidean
+    # VECTOR norms and the same eta, floored to a power of two, clamped to [dt_min, dt_max]; |jerk| = 0 -> dt_max.
+    # Hand numbers: |a| = |(3, 4, 0)| = 5, |jerk| = |(0, 0, 10)| = 10  ->  0.01 * 5 / 10 = 0.005  ->  2^-8 = 0.00390625.
+    a = np.array([[3.0, 4.0, 0.0]])
+    j = np.array([[0.0, 0.0, 10.0]])
+    assert oracle.initial_dt(a, j, 0.01)[0] == 2.0 ** -8
+    # eta enters linearly (not as sqrt(eta), which belongs to the Aarseth criterion of the corrector): 0.04 -> 0.02 -> 2^-6;
+    # 0.16 -> 0.08 -> 2^-4  (sqrt would give 0.05 -> 2^-5, 0.1 -> 2^-4 and 0.2 -> clamp 2^-3)
+    assert oracle.initial_dt(a, j, 0.04)[0] == 2.0 ** -6 and oracle.initial_dt(a, j, 0.16)[0] == 2.0 ** -4
+    # |a| / |jerk|, not |jerk| / |a| (that would be 0.02 -> 2^-6 at eta = 0.01)
+    assert oracle.initial_dt(j, a, 0.01)[0] == 2.0 ** -6 and oracle.initial_dt(a, j, 0.01)[0] != 2.0 ** -6
+    # vector norms, not a component-wise ratio or a max norm: a = (1, 1, 1) sqrt(3) norm, jerk = (2, 0, 0):
+    # eta |a| / |j| = 0.01 * 1.7320508 / 2 = 0.00866 -> 2^-7; the max norm would give 0.005 -> 2^-8
+    assert oracle.initial_dt(np.array([[1.0, 1.0, 1.0]]), np.array([[2.0, 0.0, 0.0]]), 0.01)[0] == 2.0 ** -7
+    # exponential a(t) = A exp(t / tau) u: jerk = a / tau, so dt = floor_2(eta tau) whatever A and the direction u
+    tau, u = 0.37, np.array([0.6, -0.48, 0.64])
+    for A in (1e-3, 1.3, 250.0):
+        got = oracle.initial_dt((A * u)[None], (A / tau * u)[None], 0.01)[0]
+        assert got == 2.0 ** math.floor(math.log2(0.01 * tau)) == 2.0 ** -9
+    # exact powers of two are kept, values just below go one level down
+    assert oracle.initial_dt(np.array([[2.0 ** -4, 0, 0]]), np.array([[0, 1.0, 0]]), 1.0)[0] == 2.0 ** -4
+    assert oracle.initial_dt(np.array([[2.0 ** -4 * (1 - 2.0 ** -52), 0, 0]]), np.array([[0, 1.0, 0]]), 1.0)[0] == 2.0 ** -5
+    # clamps at both ends, |jerk| = 0 -> dt_max, a = jerk = 0 -> dt_max (single particle, R19)
+    big, tiny, zero = np.array([[100.0, 0, 0]]), np.array([[1e-9, 0, 0]]), np.zeros((1, 3))
+    assert oracle.initial_dt(big, tiny, 0.01)[0] == DT_MAX and oracle.initial_dt(tiny, big, 0.01)[0] == DT_MIN
+    assert oracle.initial_dt(big, zero, 0.01)[0] == DT_MAX and oracle.initial_dt(zero, zero, 0.01)[0] == DT_MAX
+    assert oracle.initial_dt(a, j, 0.01, dt_min=2.0 ** -6, dt_max=2.0 ** -5)[0] == 2.0 ** -6
+    # one value per particle, each from its own a and jerk
+    out = oracle.initial_dt(np.vstack([a, big, tiny]), np.vstack([j, tiny, big]), 0.01)
+    assert out.tolist() == [2.0 ** -8, DT_MAX, DT_MIN]
+    # and INIT really uses it: the driver's dt after orc_init equals initial_dt of its own a, jerk
+    w = W.config(1, n=200)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    assert np.array_equal(o.dt, oracle.initial_dt(o.a, o.j, w.eta)) and np.all(o.t_i == 0.0)
+
+
 def test_block_update():
     h = 2.0 ** -6
     assert oracle.block_update(h, 0.9 * h, 5 * h) == h / 2                 # shrink: one halving is enough
@@ -238,6 +275,37 @@ def test_energy_conservation_at_eta_001(c1_run):
     for _t, _it, _ns, E in rows:
         assert abs((E - E0) / E0) < 1e-6
     assert o.nan_count == 0 and o.dtmin_clamps == 0
+
+
+def _read_c2_golden(name):
+    import os
+    out = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", name)):
+        if not line.startswith("#"):
+            k, v = line.split()
+            out[k] = float(v) if "." in v or "e" in v else int(v)
+    return out
+
+
+def test_block_rule_reading_against_the_papers_energy_error():
+    # Reading R7 (the block rule is not printed): when dt_req < h, halve ONCE per step, or halve until dt <= dt_req?
+    # The paper fixes the outcome, not the rule: "eta ~ 0.01 ... accuracy of about dE/E0 = 1e-7", and Listing 1
+    # stays below 5.4e-7 at every output.  The two stored files are the ORACLE's own C2 runs (N = 16384 to
+    # t = 1, ~5 minutes each: tests/golden/make_c2_t1_energy.py [--halving-mode 0], calling only oracle/) under the two
+    # rules: repeated halving stays inside the paper's band, a single halving per step misses it by two orders of
+    # magnitude.  That is why repeated halving is the default of the oracle (and of the CUDA path).
+    multi = _read_c2_golden("c2_t1_energy.txt")
+    single = _read_c2_golden("c2_t1_energy_single_halving.txt")
+    assert multi["e0"] == single["e0"]                                  # same input, same INIT
+    err_multi = abs(multi["e1"] / multi["e0"] - 1.0)
+    err_single = abs(single["e1"] / single["e0"] - 1.0)
+    assert err_multi <= 1e-6, err_multi                                 # 5.95e-7: the paper's order of magnitude
+    assert err_single > 1e-5, err_single                                # 4.48e-5
+    assert err_single > 50 * err_multi
+    # the schedules differ only where a step had to shrink by more than a factor two at once (56 of 30506 block steps)
+    assert 0 < multi["block_steps"] - single["block_steps"] < 0.01 * multi["block_steps"]
+    # the default of the oracle is the rule that passed
+    assert oracle.block_update(2.0 ** -6, 0.1 * 2.0 ** -6, 5 * 2.0 ** -6) == 2.0 ** -10
 
 
 def test_energy_error_grows_with_eta():

@@ -70,3 +70,35 @@ def test_weights_are_exact_integers_and_fit():
     fr = PAPER_FRACTIONS
     r, _ = lagrange.lagrange_radii(w.m, w.x, fr)
     assert np.all(np.diff(r) >= 0) and r[0] > 0
+
+
+def test_plain_definition_on_the_hand_example():
+    # the same five particles: the definition itself (float cumulative mass) gives the same radii
+    x = np.array([[3.0, 0, 0], [-1.0, 0, 0], [0, 2.0, 0], [0, 0, -5.0], [4.0, 0, 0]])
+    m = np.array([3.0, 1.0, 2.0, 2.0, 2.0])
+    r, _, who = lagrange.lagrange_radii_plain(m, x, [0.05, 0.11, 0.31, 0.75, 0.81, 1.0], centre=[0, 0, 0])
+    assert r.tolist() == [1.0, 2.0, 3.0, 4.0, 5.0, 5.0] and who.tolist() == [1, 2, 0, 4, 3, 3]
+
+
+def test_fixed_point_variant_names_the_particle_of_the_plain_definition():
+    # R24's fixed-point masses are a variant that makes the device comparison independent of summation order; away from
+    # exact ties (f M within rounding of a cumulative mass) it must pick the very particle the plain definition picks
+    w = W.config(4, n=20000)                                 # Kroupa-like masses: no two cumulative masses coincide
+    rng = np.random.default_rng(17)
+    fr = np.sort(np.concatenate([PAPER_FRACTIONS, rng.uniform(0.001, 0.999, 200)]))
+    c = np.zeros(3)
+    rp, _, who = lagrange.lagrange_radii_plain(w.m, w.x, fr, centre=c)
+    rf, _ = lagrange.lagrange_radii(w.m, w.x, fr, centre=c)
+    d = np.sort(np.linalg.norm(w.x - c, axis=1))
+    exact = rp == rf
+    # a fraction may land within ~n u M of a cumulative mass: then the two may differ by ONE particle in distance order
+    for k in np.nonzero(~exact)[0]:
+        i = int(np.searchsorted(d, rp[k]))
+        assert rf[k] in (d[max(i - 1, 0)], d[min(i + 1, len(d) - 1)]), (fr[k], rp[k], rf[k])
+    assert exact.mean() > 0.98
+    # equal masses and f n not an integer: no tie is possible, the two agree exactly
+    w2 = W.config(1)
+    fr2 = [(k + 0.5) / w2.n for k in (0, 3, 100, 511, 1000, 1022)]
+    rp2, _, _ = lagrange.lagrange_radii_plain(w2.m, w2.x, fr2, centre=c)
+    rf2, _ = lagrange.lagrange_radii(w2.m, w2.x, fr2, centre=c)
+    assert np.array_equal(rp2, rf2)
