@@ -36,6 +36,7 @@ if str(ROOT) not in sys.path:
     sys.path.insert(0, str(ROOT))
 
 FLOP_PER_PAIR = 60.0                      # BASELINE.json convention
+ENERGY_FP64_INSTR_PER_PAIR = 13.0         # k_energy_pairs: 3 DADD + 3 DFMA + 5 (rsqrt refinement) + DMUL + DFMA
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x DFMA lanes/clk/SM x 2 flop x max SM clock = 37.2
 METRIC = "fp64_hermite_force_jerk_interactions_per_s"
 UNIT = "interactions/s"
@@ -52,6 +53,7 @@ def parse_args():
     ap.add_argument("--t-end", type=float, default=None, help="override the end time (experiments only)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the C3 force-kernel sweep (extra key)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-c4", action="store_true", help="skip the bounded C4 segment (extra key)")
     ap.add_argument("--no-stages", action="store_true", help="skip the memory-bound stage timing at C5 size (extra key)")
     ap.add_argument("--only-stages", action="store_true", help="run only the memory-bound stage timing (for ncu captures)")
     return ap.parse_args()
@@ -196,9 +198,15 @@ def stage_bandwidth(gd, torch, W):
     all-active, so the corrector streams all N.  One warm-up step, then one step timed launch by launch with CUDA
     events (extra key, not `value`)."""
     w = W.config(5)
-    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
-    peak, src = hbm_peak_gbs()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    m_d, x_d, v_d = (torch.from_numpy(u).cuda() for u in (w.m, w.x, w.v))
+    torch.cuda.synchronize()
+    e0.record()
+    h = gd.Hermite(m_d, x_d, v_d, w.eps, w.eta)      # a0: pack, ONE all-active force+jerk evaluation (N^2 pairs), initial dt
+    e1.record()
+    torch.cuda.synchronize()
+    init_s = e0.elapsed_time(e1) * 1e-3
+    peak, src = hbm_peak_gbs()
 
     def timed(fn, reps=1):
         torch.cuda.synchronize()
@@ -216,6 +224,8 @@ def stage_bandwidth(gd, torch, W):
     rows["next_block"] = {"us": round(s_nb * 1e6, 2), "n_act": n_first, "algorithmic_bytes": 16.0 * w.n + 4.0 * n_first,
                           "gbs": (16.0 * w.n + 4.0 * n_first) / s_nb / 1e9, "frac_hbm": (16.0 * w.n + 4.0 * n_first) / s_nb / 1e9 / peak,
                           "note": "per call, including the device-to-host copy of (t_next, n_act) and the stream synchronisation"}
+    h.energy()                                         # a6 at this size (warm-up call, then one timed call)
+    sec_en, _ = timed(h.energy)
     h.set_option("dt_level_min", 10)
     h.set_option("dt_level_max", 10)
     samples = {"next_block_all_active": [], "predictor": [], "corrector_timestep": []}
@@ -235,8 +245,64 @@ def stage_bandwidth(gd, torch, W):
                       "frac_hbm": nbytes / sec / 1e9 / peak}
     h.close()
     rows["next_block_all_active"]["note"] = rows["next_block"]["note"] + "; 4 B of index written per active particle"
-    return {"workload": f"C5 size N={w.n}, shared step 2^-10 (all-active block steps), median of three steps after a warm-up step; "
+    # the predictor's writes (56 B per particle) stay in L2 over back-to-back launches: its DRAM side is the 128 B read
+    rows["predictor"]["dram_side_bytes"] = 128.0 * w.n
+    rows["predictor"]["frac_hbm_reads_only"] = 128.0 * w.n / (rows["predictor"]["us"] * 1e-6) / 1e9 / peak
+    all_active = {"n": w.n, "ms": init_s * 1e3, "tflops60": FLOP_PER_PAIR * float(w.n) * w.n / init_s / 1e12,
+                  "frac_fp64_nominal": FLOP_PER_PAIR * float(w.n) * w.n / init_s / 1e12 / FP64_NOMINAL_TFLOPS,
+                  "what": "gd_init on C5 (N = 2^20 + 1): pack + one all-active k_force_ipar evaluation + initial dt, CUDA events"}
+    # a6 at this size: N (N - 1) / 2 softened pair potentials + N kinetic terms per call (the predictor runs first)
+    pairs_en = 0.5 * float(w.n) * (w.n - 1)
+    energy = {"n": w.n, "ms": sec_en * 1e3, "pairs_per_s": pairs_en / sec_en,
+              "fp64_instr_per_pair": ENERGY_FP64_INSTR_PER_PAIR,
+              "frac_fp64_issue": pairs_en * ENERGY_FP64_INSTR_PER_PAIR * 2.0 / sec_en / 1e12 / FP64_NOMINAL_TFLOPS,
+              "what": "gd_energy (k_predict + k_energy_pairs + k_energy_reduce + D2H of K, U), one call, CUDA events; fraction = "
+                      "pairs x 13 FP64 instructions x 2 flop slots / time / nominal FP64 peak"}
+    return {"all_active": all_active, "energy": energy, "workload": f"C5 size N={w.n}, shared step 2^-10 (all-active block steps), median of three steps after a warm-up step; "
                         "predictor: 10 back-to-back launches", "hbm_peak_gbs": peak, "hbm_peak_source": src, "stages": rows}
+
+
+def c4_segment(gd, torch, W, t_seg=0.125):
+    """C4 (BASELINE.json configs[3]: N = 262144, Kroupa-like masses): gd_init event-timed (one all-active evaluation at
+    this N), then a bounded segment of its block-step integration -- t = 0 to the first synchronisation time dt_max =
+    0.125, half of the config's t = 0.25 -- with the wall time per N-body time unit and the per-level histogram the
+    config asks for (extra key, not `value`)."""
+    w = W.config(4)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    m_d, x_d, v_d = (torch.from_numpy(u).cuda() for u in (w.m, w.x, w.v))
+    torch.cuda.synchronize()
+    e0.record()
+    h = gd.Hermite(m_d, x_d, v_d, w.eps, w.eta)
+    e1.record()
+    torch.cuda.synchronize()
+    init_s = e0.elapsed_time(e1) * 1e-3
+    k0, u0 = h.energy()
+    e0.record()
+    steps, psteps = h.run_until(t_seg)
+    e1.record()
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3
+    k1, u1 = h.energy()
+    hist, diag = h.level_histogram()
+    lp = h.loop_profile()
+    sizes = h.loop_histogram()
+    h.close()
+    pairs = float(psteps) * w.n
+    return {
+        "all_active": {"n": w.n, "ms": init_s * 1e3, "tflops60": FLOP_PER_PAIR * float(w.n) * w.n / init_s / 1e12,
+                       "frac_fp64_nominal": FLOP_PER_PAIR * float(w.n) * w.n / init_s / 1e12 / FP64_NOMINAL_TFLOPS,
+                       "what": "gd_init on C4 (N = 262144): pack + one all-active k_force_ipar evaluation + initial dt, CUDA events"},
+        "segment": {"workload": f"C4: {w.name}, eps={w.eps}, eta={w.eta}, block steps t = 0 .. {t_seg} (the first dt_max interval "
+                                "of the config's t = 0.25)", "n": w.n, "t_end": t_seg, "ms": sec * 1e3,
+                    "wall_s_per_nbody_time_unit": sec / t_seg, "block_steps": steps, "particle_steps": psteps,
+                    "interactions_per_s": pairs / sec, "tflops60": FLOP_PER_PAIR * pairs / sec / 1e12,
+                    "frac_fp64_nominal": FLOP_PER_PAIR * pairs / sec / 1e12 / FP64_NOMINAL_TFLOPS,
+                    "steps_inside_persistent_loop": lp["block_steps"],
+                    "energy_rel_err": abs((k1 + u1) / (k0 + u0) - 1.0),
+                    "particle_steps_per_level": {str(k): int(c) for k, c in enumerate(hist) if c},
+                    "dt_min_clamps": int(diag[1]), "nan_criteria": int(diag[0]),
+                    "block_steps_by_active_set_size": [{"n_act_below": r["n_act_below"], "block_steps": r["block_steps"],
+                                                        "particle_steps": r["particle_steps"]} for r in sizes]}}
 
 
 def cpu_sample_steps(n: int) -> int:
@@ -256,6 +322,57 @@ def cpu_baseline(w, t_end):
     return {"value": pairs / sec, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
             "sample": f"{w.name}: INIT (N^2 pairs) + first {o.block_steps} block steps "
                       f"({o.particle_steps} particle steps, to t={o.t:.6g}); plain FP64 sums; {sec:.1f} s"}, sec
+
+
+def cpu_table(W):
+    """the oracle's all-active PAIRSUM rate, single-thread and all cores, at the five sizes (a
+    seeded subset of sinks against all N sources where N^2 would take minutes: "subset"), and the share of the
+    oracle's block-step run spent in the force sums (the paper: ~95 %).  About 20 s of host work."""
+    import numpy as np
+    import oracle
+    cores = oracle.num_threads()
+    rows = []
+    for cfg, n_one, n_all in ((1, 1024, 1024), (2, 1024, 8192), (3, 512, 4096), (4, 256, 2048), (5, 128, 1024)):
+        w = W.config(cfg)
+        row = {"config": f"C{cfg}", "n": w.n}
+        for label, k, threads in (("single_thread", n_one, 1), ("all_cores", n_all, cores)):
+            k = min(k, w.n)
+            idx = None if k == w.n else np.sort(np.random.default_rng(1000 + cfg).choice(w.n, k, replace=False)).astype(np.int32)
+            oracle.set_num_threads(threads)
+            oracle.pairsum(w.m[:64], w.x[:64], w.v[:64], w.eps, mode="plain")      # the thread team exists before the clock starts
+            t0 = time.perf_counter()
+            oracle.pairsum(w.m, w.x, w.v, w.eps, idx=idx, mode="plain")
+            sec = time.perf_counter() - t0
+            row[label] = {"interactions_per_s": k * float(w.n) / sec, "sinks": k, "seconds": round(sec, 3),
+                          "sample": "full N^2" if k == w.n else f"subset: {k} seeded sinks x all N sources"}
+        oracle.set_num_threads(cores)
+        rows.append(row)
+    # force share of a block-step run: C1 (N = 1024) to t = 0.125 in full, the oracle's own timers
+    w = W.config(1)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta, acc_mode="plain")
+    o.run(0.125)
+    f, tot = o.seconds
+    oracle.set_num_threads(1)
+    o1 = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta, acc_mode="plain")
+    o1.run(0.125)
+    f1, tot1 = o1.seconds
+    oracle.set_num_threads(cores)
+    return {"cores": cores, "kind": "oracle", "rows": rows,
+            "force_share_of_block_step_run": {"workload": "C1 N=1024 to t=0.125 (INIT + %d block steps)" % o.block_steps,
+                                              "all_cores": f / tot, "single_thread": f1 / tot1,
+                                              "seconds_all_cores": tot, "seconds_single_thread": tot1,
+                                              "paper": "~0.95 on a serial CPU build (P:161)"}}
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """dram bytes per launch of `kernel` from the committed `ncu --set full` capture, if profiles/ncu_traffic.json holds
+    one for this workload and kernel: {"<workload>/<kernel>": {"dram_bytes": ..., "profile": "profiles/...", "commit": ...}}.
+    A capture is a property of the commit it was taken at, so the entry names it; no entry -> None."""
+    try:
+        ent = json.loads((ROOT / "profiles" / "ncu_traffic.json").read_text()).get(f"{workload}/{kernel}")
+    except (OSError, ValueError):
+        ent = None
+    return (ent.get("dram_bytes"), ent) if ent else (None, None)
 
 
 def aggregate_replicas(torch, dist, device, sec, sec_e2e, pairs, pairs_e2e):
@@ -346,10 +463,6 @@ def main_ours(args):
                        clocks.summary(), prof_pass)
 
 
-# dram bytes per launch of the dominant force kernel from the committed `ncu --set full` capture under profiles/
-# (None until one exists for the workload)
-NCU_TRAFFIC_BYTES = {("C2", "jsplit"): 938240, ("C2", "ipar"): 934656, ("C2", "ipar_small"): 936192,   # profiles/r1c_launches_graph_path.md
-                     ("C2", "loop"): 14877042000}                                                # profiles/r1r_final_round1.md
 KERNEL_NAMES = {"ipar": "k_force_ipar<2,1>", "jsplit": "k_force_jsplit", "ipar_small": "k_force_ipar<1,4>",
                 "loop": "k_block_loop", "slice": "k_force_slice"}
 
@@ -366,7 +479,8 @@ def finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, 
     roofline = {
         "bound": "alu", "kernel": KERNEL_NAMES[dom],
         "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
-        "traffic": NCU_TRAFFIC_BYTES.get((args.workload, dom)),
+        "traffic": ncu_traffic(args.workload, KERNEL_NAMES[dom])[0],
+        "traffic_source": ncu_traffic(args.workload, KERNEL_NAMES[dom])[1],
         "peak_source": "derived: 148 SM x 64 DFMA lanes/clk x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
                        "entry); register-only DFMA probe on this box: %.2f TFLOP/s" % (peak_probe / 1e12),
         "launches": int(d["launches"]), "avg_launch_us": 1e3 * d["ms"] / max(d["launches"], 1),
@@ -413,12 +527,27 @@ def finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, 
         "mean_n_act": r0["particle_steps"] / max(r0["block_steps"], 1),
         "energy": {"e0": r0["e0"], "e1": r0["e1"], "rel_err": abs(r0["e1"] / r0["e0"] - 1.0)},
     }
+    all_active = []
     if not args.no_sweep:
         line["force_sweep"] = force_sweep(gd, torch, W)
+        p = line["force_sweep"]["points"][-1]
+        all_active.append({"n": 65536, "ms": p["us"] * 1e-3, "tflops60": p["tflops60"], "frac_fp64_nominal": p["frac_fp64_nominal"],
+                           "what": "gd_force_jerk over all 65536 sinks of C3, 10 back-to-back launches, CUDA events"})
+    if not args.no_c4:
+        c4 = c4_segment(gd, torch, W)
+        all_active.append(c4["all_active"])
+        line["c4_segment"] = c4["segment"]
     if not args.no_stages:
-        line["memory_bound_stages"] = stage_bandwidth(gd, torch, W)
+        st = stage_bandwidth(gd, torch, W)
+        all_active.append(st.pop("all_active"))
+        line["energy_a6"] = st.pop("energy")
+        line["memory_bound_stages"] = st
+    if all_active:
+        # north_star: "the all-active force/jerk kernel sustains >= 70 % of B200 FP64 peak at N >= 65536"
+        line["all_active"] = all_active
     if not args.no_cpu and world == 1:
         line["cpu_baseline"], _ = cpu_baseline(w, t_end)
+        line["cpu_baseline"]["table"] = cpu_table(W)
     print(json.dumps(line), flush=True)
     return line
 

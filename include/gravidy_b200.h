@@ -15,7 +15,11 @@
  *   - All floating point is IEEE binary64.  Indices are int32.  G = 1 (N-body units).
  *   - Pointers named *_dev are DEVICE pointers, *_host are HOST pointers.  The library never allocates
  *     device memory: the caller hands one workspace of gd_workspace_bytes(n) bytes (256-byte aligned) to
- *     gd_init and keeps it alive until gd_destroy.  Inputs are copied at init and may be freed afterwards.
+ *     gd_init and keeps it alive until gd_destroy.  Inputs are copied at init: HOST inputs (gd_init_host) may be
+ *     reused or freed as soon as the call returns (it synchronises once the copies are done); DEVICE inputs (gd_init)
+ *     are read by a kernel enqueued on the stream and must stay untouched until the stream has passed it (any
+ *     synchronising call, or stream order).  (The two self-tests gd_fp64_peak_probe / gd_selftest_div_const, which
+ *     take no ctx, allocate and free 8 bytes of their own.)
  *   - [n,3] arrays are row-major (x0 y0 z0 x1 y1 z1 ...).
  *   - All work is enqueued on the CUDA stream given at init (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream).  Calls are asynchronous unless stated; the ones that return values to the
@@ -70,7 +74,8 @@ GD_API int gd_init(gd_ctx **out, int64_t n, const double *m_dev, const double *x
             double eps, double eta, void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
 
 /* Same as gd_init with HOST input arrays (pageable or pinned): the host->device copies are part of the
- * call.  Used for end-to-end timing. */
+ * call, and the call waits for them (and for the kernel that repacks them) before it returns, so the arrays may be
+ * reused at once; the all-active force evaluation behind them stays asynchronous.  Used for end-to-end timing. */
 GD_API int gd_init_host(gd_ctx **out, int64_t n, const double *m_host, const double *x_host, const double *v_host,
                  double eps, double eta, void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
 

@@ -8,3 +8,4 @@ from .oracle import (  # noqa: F401
     block_update, initial_dt, num_threads, set_num_threads, DT_MAX, DT_MIN,
 )
 from . import lagrange  # noqa: F401,E402
+from . import structure  # noqa: F401,E402

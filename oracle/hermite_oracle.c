@@ -28,6 +28,7 @@
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#include <time.h>
 #ifdef _OPENMP
 #include <omp.h>
 #endif
@@ -319,7 +320,15 @@ typedef struct {
     int64_t diag[2];                        /* NaN criteria, dt_min clamps */
     double min_margin;                      /* closest approach of dt_req to a decision threshold */
     int64_t level_hist[64];                 /* particle steps taken with dt = 2^-k */
+    double sec_force, sec_total;            /* wall seconds inside PAIRSUM / inside orc_init + orc_step ("95 %") */
 } orc_state;
+
+static double orc_now(void)
+{
+    struct timespec ts;
+    clock_gettime(CLOCK_MONOTONIC, &ts);
+    return (double)ts.tv_sec + 1e-9 * (double)ts.tv_nsec;
+}
 
 ORC_API int64_t orc_state_size(void) { return (int64_t)sizeof(orc_state); }
 
@@ -330,18 +339,25 @@ ORC_API void orc_init(orc_state *s)
     s->diag[0] = s->diag[1] = 0;
     s->min_margin = INFINITY;
     memset(s->level_hist, 0, sizeof(s->level_hist));
+    double w0 = orc_now();
     orc_pairsum(s->n, s->m, s->x, s->v, s->eps2, NULL, s->n, s->a, s->j, s->acc_mode);
+    double w1 = orc_now();
     orc_initial_dt(s->n, s->a, s->j, s->eta, s->dt_min, s->dt_max, s->dt);
     for (int64_t i = 0; i < s->n; ++i) s->t_i[i] = 0.0;
     s->n_act = 0;
+    s->sec_force = w1 - w0;
+    s->sec_total = orc_now() - w0;
 }
 
 /* One block step.  Returns the new time. */
 ORC_API double orc_step(orc_state *s)
 {
+    double w0 = orc_now();
     double tn = orc_next_block(s->n, s->t_i, s->dt, s->active, &s->n_act);
     orc_predict(s->n, tn, s->x, s->v, s->a, s->j, s->t_i, s->xp, s->vp);
+    double w1 = orc_now();
     orc_pairsum(s->n, s->m, s->xp, s->vp, s->eps2, s->active, s->n_act, s->a1, s->j1, s->acc_mode);
+    s->sec_force += orc_now() - w1;
     for (int64_t k = 0; k < s->n_act; ++k) {
         int e;
         (void)frexp(s->dt[s->active[k]], &e);    /* dt = 2^(e-1) */
@@ -353,6 +369,7 @@ ORC_API double orc_step(orc_state *s)
     s->t = tn;
     s->block_steps += 1;
     s->particle_steps += s->n_act;
+    s->sec_total += orc_now() - w0;
     return tn;
 }
 

@@ -53,6 +53,7 @@ class _State(C.Structure):
         ("diag", C.c_int64 * 2),
         ("min_margin", C.c_double),
         ("level_hist", C.c_int64 * 64),
+        ("sec_force", C.c_double), ("sec_total", C.c_double),
     ]
 
 
@@ -266,6 +267,11 @@ class HermiteOracle:
     @property
     def min_margin(self) -> float:
         return float(self._s.min_margin)
+
+    @property
+    def seconds(self) -> tuple[float, float]:
+        """(wall seconds inside PAIRSUM, wall seconds inside INIT + the block steps) so far (force ~ 95 %)."""
+        return float(self._s.sec_force), float(self._s.sec_total)
 
     @property
     def level_hist(self) -> np.ndarray:

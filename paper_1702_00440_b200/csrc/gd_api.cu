@@ -71,10 +71,17 @@ static inline int64_t gd_pad(int64_t n) { return ((n + GD_TILE_J - 1) / GD_TILE_
 // GD_LP_MAX_NP particles) keeps one row per (CTA, active particle), for up to GD_LP_GRID_BOUND CTAs
 #define GD_LP_MAX_NP (1 << 19)
 #define GD_LP_GRID_BOUND 160
+// largest active set the loop's scratch is sized for.  The whole system: measured on C4 (N = 262144, t = 0 .. 2^-5), with
+// the steps above 32768 sinks handed to the stage kernels behind the loop the run took 10.5 s instead of 2.9 s (the 33
+// largest steps cost 280 ms each outside the loop, 51 ms inside), so every step stays inside.
+#ifndef GD_LP_MAX_HI
+#define GD_LP_MAX_HI GD_LP_MAX_NP
+#endif
 static inline int64_t gd_pcap(int64_t np)
 {
     int64_t r = (4 * np > (1 << 20)) ? 4 * np : (1 << 20);
-    if (np <= GD_LP_MAX_NP && GD_LP_GRID_BOUND * np > r) r = GD_LP_GRID_BOUND * np;
+    const int64_t hi = np < GD_LP_MAX_HI ? np : GD_LP_MAX_HI;
+    if (np <= GD_LP_MAX_NP && GD_LP_GRID_BOUND * hi > r) r = GD_LP_GRID_BOUND * hi;
     return r;
 }
 static inline size_t gd_up(size_t b) { return (b + 255) & ~(size_t)255; }
@@ -160,8 +167,12 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
 {
     if (!out) return gd_fail(nullptr, GD_EINVAL, "gd_init: out is NULL");
     *out = nullptr;
-    if (n < 1 || n > (int64_t)1 << 30) return gd_fail(nullptr, GD_EINVAL, "gd_init: n out of range");
+    // the active-set compaction scans at most GD_SCAN_MAX_BLOCKS x 32 rounds x GD_SCAN_THREADS particles
+    if (n < 1 || n > (int64_t)GD_SCAN_MAX_BLOCKS * 32 * GD_SCAN_THREADS) return gd_fail(nullptr, GD_EINVAL, "gd_init: n out of range (1 .. 2^25)");
     if (!(eta > 0.0) || !(eps >= 0.0) || !isfinite(eta) || !isfinite(eps)) return gd_fail(nullptr, GD_EINVAL, "gd_init: need eta > 0 and eps >= 0");
+    // eps > 0 keeps the self pair in the sum (m / eps^3 times a zero vector): eps^3 must not underflow the pair term to
+    // inf * 0.  Below 1e-100 only eps == 0 (the masked path) is accepted.
+    if (eps > 0.0 && eps < 1e-100) return gd_fail(nullptr, GD_EINVAL, "gd_init: eps must be 0 or >= 1e-100");
     if (!ws || ((uintptr_t)ws & 255)) return gd_fail(nullptr, GD_EINVAL, "gd_init: workspace NULL or not 256-byte aligned");
     if (ws_bytes < gd_workspace_bytes(n)) return gd_fail(nullptr, GD_EINVAL, "gd_init: workspace too small (see gd_workspace_bytes)");
     gd_ctx *c = (gd_ctx *)calloc(1, sizeof(gd_ctx));
@@ -180,7 +191,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->use_graph = 1;
     c->jsplit_max_nact = 512;
     c->ipar_small_max_nact = 2048;
-    c->loop_max_nact = (int64_t)1 << 40;      // every step the scratch allows
+    c->loop_max_nact = GD_LP_MAX_HI;          // every step the scratch allows (larger active sets: i-parallel stage kernel)
     c->loop_small_nact = 96;
     c->loop_warp_correct = 48;
     c->slice_max_nact = 8192;
@@ -213,11 +224,14 @@ static int gd_prepare(gd_ctx *c)
     return rc;
 }
 
-static int gd_init_common(gd_ctx *c, const double *m_dev, const double *x_dev, const double *v_dev)
+static int gd_init_common(gd_ctx *c, const double *m_dev, const double *x_dev, const double *v_dev, bool wait_inputs)
 {
     int rc;
     if ((rc = gd_prepare(c))) return rc;
     if ((rc = gdk_pack_state(c, m_dev, x_dev, v_dev))) return rc;          // also the predicted records at t = 0
+    // host inputs: the caller may reuse its arrays when the call returns, so wait here -- before the O(N^2) evaluation is
+    // enqueued, not after it -- until the copies and the repacking kernel are done
+    if (wait_inputs) GD_CUDA(c, cudaStreamSynchronize(c->stream));
     c->t = 0.0;
     c->t_pred = 0.0;
     c->have_pred = true;
@@ -235,8 +249,8 @@ extern "C" int gd_init(gd_ctx **out, int64_t n, const double *m_dev, const doubl
     if (!m_dev || !x_dev || !v_dev) return gd_fail(nullptr, GD_EINVAL, "gd_init: NULL input array");
     int rc = gd_create(out, n, eps, eta, workspace_dev, workspace_bytes, cuda_stream);
     if (rc) return rc;
-    rc = gd_init_common(*out, m_dev, x_dev, v_dev);
-    if (rc) { snprintf(g_init_err, sizeof g_init_err, "%s", (*out)->err); gd_destroy(*out); *out = nullptr; }
+    rc = gd_init_common(*out, m_dev, x_dev, v_dev, false);
+    if (rc) { cudaStreamSynchronize((*out)->stream); snprintf(g_init_err, sizeof g_init_err, "%s", (*out)->err); gd_destroy(*out); *out = nullptr; }
     return rc;
 }
 
@@ -251,8 +265,8 @@ extern "C" int gd_init_host(gd_ctx **out, int64_t n, const double *m_host, const
     cudaError_t e = cudaMemcpyAsync(st, m_host, n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(st + c->np, x_host, 3 * n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(st + 4 * c->np, v_host, 3 * n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
-    rc = (e == cudaSuccess) ? gd_init_common(c, st, st + c->np, st + 4 * c->np) : gd_fail_cuda(c, e, "gd_init_host: H2D copy");
-    if (rc) { snprintf(g_init_err, sizeof g_init_err, "%s", c->err); gd_destroy(c); *out = nullptr; }
+    rc = (e == cudaSuccess) ? gd_init_common(c, st, st + c->np, st + 4 * c->np, true) : gd_fail_cuda(c, e, "gd_init_host: H2D copy");
+    if (rc) { cudaStreamSynchronize(c->stream); snprintf(g_init_err, sizeof g_init_err, "%s", c->err); gd_destroy(c); *out = nullptr; }
     return rc;
 }
 
@@ -296,7 +310,9 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
         int lo = !strcmp(key, "dt_level_min") ? lv : c->lvl_min, hi = !strcmp(key, "dt_level_max") ? lv : c->lvl_max;
         c->lvl_min = lo;
         c->lvl_max = hi;
-        if (lo > hi) return GD_OK;                 // transient while the caller sets both; checked below once ordered
+        c->have_block = c->have_force = c->have_pred = false;   // any active list / force result in flight is void now
+        gd_graph_drop(c);
+        if (lo > hi) return GD_OK;                 // transient while the caller sets both: every stage call fails with GD_ESTATE until ordered
         c->dt_max = ldexp(1.0, -lo);
         c->dt_min = ldexp(1.0, -hi);
         gd_graph_drop(c);
@@ -332,6 +348,7 @@ extern "C" int gd_predict(gd_ctx *c, double t)
 {
     if (!c) return GD_EINVAL;
     if (t != t) return gd_fail(c, GD_EINVAL, "gd_predict: t is NaN");
+    if (c->lvl_min > c->lvl_max) return gd_fail(c, GD_ESTATE, "gd_predict: dt_level_min > dt_level_max");
     int rc = gdk_predict(c, t);
     if (rc) return rc;
     c->t_pred = t;
@@ -343,6 +360,7 @@ extern "C" int gd_predict(gd_ctx *c, double t)
 extern "C" int gd_force_jerk(gd_ctx *c, const int32_t *idx_dev, int64_t n_act, double *a_out_dev, double *j_out_dev)
 {
     if (!c) return GD_EINVAL;
+    if (c->lvl_min > c->lvl_max) return gd_fail(c, GD_ESTATE, "gd_force_jerk: dt_level_min > dt_level_max");
     if (!c->have_pred) return gd_fail(c, GD_ESTATE, "gd_force_jerk: no predicted records (call gd_predict first)");
     if ((a_out_dev == nullptr) != (j_out_dev == nullptr)) return gd_fail(c, GD_EINVAL, "gd_force_jerk: give both outputs or neither");
     if (!idx_dev) {
@@ -360,6 +378,7 @@ extern "C" int gd_force_jerk(gd_ctx *c, const int32_t *idx_dev, int64_t n_act, d
 extern "C" int gd_correct_and_timestep(gd_ctx *c)
 {
     if (!c) return GD_EINVAL;
+    if (c->lvl_min > c->lvl_max) return gd_fail(c, GD_ESTATE, "gd_correct_and_timestep: dt_level_min > dt_level_max");
     if (!c->have_block || !c->have_force)
         return gd_fail(c, GD_ESTATE, "gd_correct_and_timestep: needs gd_next_block, gd_predict(t_next), gd_force_jerk(NULL) first");
     int rc = gdk_correct(c, c->t_next);
