@@ -179,6 +179,19 @@ GD_API int gd_get_level_histogram(gd_ctx *ctx, int64_t *counts_host, int64_t *di
  * order of summation (R24).  On-device 8-pass radix select, no sort.  Synchronises. */
 GD_API int gd_lagrange_radii(gd_ctx *ctx, const double *center_host, const double *fractions_host, int n_frac,
                              double *radii_host, double *center_out_host);
+/* Time-step census, "the distribution of the time steps" (Fig. 13 P:363 shows it at four times): counts_host[64]
+ * <- the number of particles whose CURRENT block step is 2^-k, k = 0 .. 63 (gd_get_level_histogram counts the particle
+ * steps TAKEN per level since init instead).  Synchronises. */
+GD_API int gd_get_level_census(gd_ctx *ctx, int64_t *counts_host);
+/* Density centre and core radius, "the core radius as calculated at T=0" (Fig. 12).  The paper prints no
+ * definition; reading R25 takes Casertano & Hut (1985) as the direct-summation codes use it: with r_iK the
+ * distance from particle i to its K-th nearest neighbour (K = k_neighbours, 2 .. 8; 6 is the usual choice),
+ *   rho_i = (sum of the masses of the K - 1 nearest neighbours) / (4 pi / 3 r_iK^3)
+ *   x_d = sum rho_i x_i / sum rho_i ;   r_c = sqrt( sum rho_i^2 |x_i - x_d|^2 / sum rho_i^2 )
+ * on the positions predicted to the current time.  *core_radius_host <- r_c; density_centre_host: NULL or HOST [3] <- x_d;
+ * rho_dev: NULL or a DEVICE array [n] that receives rho_i.  O(n^2) distance evaluations on the device (every particle
+ * keeps its K nearest in registers).  Overwrites the predicted records like gd_energy.  Synchronises. */
+GD_API int gd_core_radius(gd_ctx *ctx, int k_neighbours, double *core_radius_host, double *density_centre_host, double *rho_dev);
 /* Counters of the persistent block-step loop (k_block_loop, the kernel behind gd_step / gd_run_until that takes the
  * block steps) since init -> out_host[11] = { particle steps, block steps taken inside
  * the loop, ns spent inside it (device global timer, CTA 0), ns in its force phase, in the barrier after it, in its

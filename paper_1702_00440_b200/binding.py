@@ -52,6 +52,8 @@ SYMBOLS = {
     "gd_get_profile": (_int, [_vp, _vp]),
     "gd_get_loop_profile": (_int, [_vp, _vp]),
     "gd_get_loop_histogram": (_int, [_vp, _vp]),
+    "gd_get_level_census": (_int, [_vp, _vp]),
+    "gd_core_radius": (_int, [_vp, _int, _pdbl, _vp, _vp]),
     "gd_lagrange_radii": (_int, [_vp, _vp, _vp, _int, _vp, _vp]),
     "gd_fp64_peak_probe": (_int, [_int, _pdbl, _pdbl]),
     "gd_selftest_div_const": (_int, [C.c_int64, C.c_uint64, _vp]),
@@ -323,6 +325,20 @@ class Hermite:
         self._check(self._lib.gd_lagrange_radii(self._h, c.ctypes.data if c is not None else None, f.ctypes.data,
                                                 int(f.shape[0]), r.ctypes.data, co.ctypes.data))
         return r, co[:3].copy(), float(co[3])
+
+    def level_census(self) -> np.ndarray:
+        """Number of particles per CURRENT block step 2^-k (Fig. 13)."""
+        h = np.zeros(64, dtype=np.int64)
+        self._check(self._lib.gd_get_level_census(self._h, h.ctypes.data))
+        return h
+
+    def core_radius(self, k: int = 6, want_rho: bool = False):
+        """(r_c, density centre[3]) or (r_c, centre, rho CUDA tensor [n]) -- Casertano & Hut (1985), R25."""
+        torch = _torch()
+        rc, xd = C.c_double(0), np.zeros(3)
+        rho = torch.empty((self.n,), dtype=torch.float64, device="cuda") if want_rho else None
+        self._check(self._lib.gd_core_radius(self._h, int(k), C.byref(rc), xd.ctypes.data, rho.data_ptr() if want_rho else None))
+        return (rc.value, xd, rho) if want_rho else (rc.value, xd)
 
     def loop_profile(self) -> dict:
         o = np.zeros(11, dtype=np.int64)

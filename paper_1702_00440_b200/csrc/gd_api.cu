@@ -429,6 +429,37 @@ extern "C" int gd_lagrange_radii(gd_ctx *c, const double *center_host, const dou
     return GD_OK;
 }
 
+extern "C" int gd_get_level_census(gd_ctx *c, int64_t *counts_host)
+{
+    if (!c || !counts_host) return GD_EINVAL;
+    unsigned long long *cnt = c->d.diag_scratch + 64;        // the histogram area of the Lagrange-radius select: free between calls
+    int rc = gdk_census(c, cnt);
+    if (rc) return rc;
+    GD_CUDA(c, cudaMemcpyAsync(counts_host, cnt, 64 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return GD_OK;
+}
+
+extern "C" int gd_core_radius(gd_ctx *c, int k_neighbours, double *core_radius_host, double *density_centre_host, double *rho_dev)
+{
+    if (!c || !core_radius_host) return GD_EINVAL;
+    if (k_neighbours < 2 || k_neighbours > 8) return gd_fail(c, GD_EINVAL, "gd_core_radius: 2 <= k_neighbours <= 8");
+    if (c->n <= k_neighbours) return gd_fail(c, GD_EINVAL, "gd_core_radius: needs more than k_neighbours particles");
+    int rc = gdk_predict(c, c->t);
+    if (rc) return rc;
+    c->t_pred = c->t;
+    c->have_pred = true;
+    c->have_force = false;
+    double *st = (double *)c->d.staging;                     // [0, 6) results
+    if ((rc = gdk_core_radius(c, k_neighbours, rho_dev, st))) return rc;
+    double out[6];
+    GD_CUDA(c, cudaMemcpyAsync(out, st, sizeof out, cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaStreamSynchronize(c->stream));
+    *core_radius_host = out[3];
+    if (density_centre_host) { density_centre_host[0] = out[0]; density_centre_host[1] = out[1]; density_centre_host[2] = out[2]; }
+    return GD_OK;
+}
+
 static int gd_one_step(gd_ctx *c)
 {
     int rc = gd_next_block(c, nullptr, nullptr);

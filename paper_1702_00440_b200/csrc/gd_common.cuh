@@ -138,6 +138,8 @@ int64_t gdk_slice_hi(const gd_ctx *c);
 int gdk_force_slice(gd_ctx *c, const int32_t *idx, int64_t n_act, double *a_out, double *j_out, bool dev);
 int gdk_energy(gd_ctx *c);
 int gdk_lagrange(gd_ctx *c, const double *center_host, const double *frac_dev, int n_frac, double *radii_dev);   // gd_diag.cu                                                                   // gd_energy.cu
+int gdk_census(gd_ctx *c, unsigned long long *counts_dev);
+int gdk_core_radius(gd_ctx *c, int K, double *rho_dev, double *out_dev);
 int gdk_selftest_div_const(long long n, unsigned long long seed, long long *mismatches);          // gd_probe.cu
 int gdk_fp64_probe(int iters, double *flops, double *ms);                                    // gd_probe.cu
 

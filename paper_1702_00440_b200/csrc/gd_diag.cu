@@ -166,3 +166,147 @@ int gdk_lagrange(gd_ctx *c, const double *center_host, const double *frac_dev, i
     }
     return 0;
 }
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// Time-step census ("the distribution of the time steps"; Fig. 13): counts[k] = number of particles whose
+// CURRENT block step is 2^-k.  (The histogram of particle steps TAKEN per level is d.hist, kept by the corrector.)
+// Integer counts: exact in any order.  Memory-bound, 32 B per particle (the {a, dt} vector); not on the hot path.
+__global__ void __launch_bounds__(GD_LG_THREADS) k_diag_census(gd_dev d, int64_t n, unsigned long long *counts)
+{
+    __shared__ unsigned int s_cnt[64];
+    if (threadIdx.x < 64) s_cnt[threadIdx.x] = 0u;
+    __syncthreads();
+    for (int64_t i = (int64_t)blockIdx.x * GD_LG_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * GD_LG_THREADS) {
+        const long long bits = __double_as_longlong(d.ad[i].w);
+        const int lvl = 1023 - (int)((bits >> 52) & 0x7ff);
+        if (bits > 0 && (bits & 0xfffffffffffffLL) == 0 && lvl >= 0 && lvl < 64) atomicAdd(&s_cnt[lvl], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x < 64 && s_cnt[threadIdx.x]) atomicAdd(&counts[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
+}
+
+int gdk_census(gd_ctx *c, unsigned long long *counts_dev)
+{
+    GD_CUDA(c, cudaMemsetAsync(counts_dev, 0, 64 * sizeof(unsigned long long), c->stream));
+    unsigned blocks = (unsigned)((c->n + GD_LG_THREADS - 1) / GD_LG_THREADS);
+    if (blocks > (unsigned)(8 * c->sm_count)) blocks = (unsigned)(8 * c->sm_count);
+    k_diag_census<<<blocks, GD_LG_THREADS, 0, c->stream>>>(c->d, c->n, counts_dev);
+    GD_LAUNCH_CHECK(c, "k_diag_census");
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// Density centre and core radius ("the core radius as calculated at T=0", Fig. 12; the paper prints no
+// definition: reading R25 = Casertano & Hut 1985 as the direct-summation codes use it):
+//   rho_i = (masses of the K - 1 nearest neighbours of i) / (4 pi / 3 r_iK^3),   r_iK = distance to the K-th nearest
+//   x_d = sum rho_i x_i / sum rho_i ;   r_c = sqrt( sum rho_i^2 |x_i - x_d|^2 / sum rho_i^2 )
+// on the positions predicted to the current time.
+// k_diag_knn: one thread per particle i, all n sources streamed through shared memory in tiles; every thread keeps the
+// K smallest squared distances seen so far (and the masses that go with them) in registers, ascending, a new source
+// entering only if strictly closer than the K-th (so equal distances keep index order).  Every operation is rounded
+// separately in the order the definition is written, so r^2, the choice of neighbours and rho_i are the doubles a
+// plain evaluation gives.  ALU-bound: n^2 x ~10 FP64 instructions; a diagnostic, not on the hot path.
+#define GD_KNN_MAXK 8
+#define GD_KNN_TILE 256
+
+__global__ void __launch_bounds__(GD_KNN_TILE) k_diag_knn(gd_dev d, int64_t n, int K, double *rho)
+{
+    __shared__ double2 s_xy[GD_KNN_TILE], s_zm[GD_KNN_TILE];
+    const int64_t i = (int64_t)blockIdx.x * GD_KNN_TILE + threadIdx.x;
+    const bool live = i < n;
+    const double2 xy = live ? d.pxy[i] : make_double2(0.0, 0.0), zm = live ? d.pzm[i] : make_double2(0.0, 0.0);
+    double r2k[GD_KNN_MAXK], mk[GD_KNN_MAXK];
+#pragma unroll
+    for (int k = 0; k < GD_KNN_MAXK; ++k) { r2k[k] = __longlong_as_double(0x7ff0000000000000LL); mk[k] = 0.0; }
+    for (int64_t j0 = 0; j0 < n; j0 += GD_KNN_TILE) {
+        const int64_t j = j0 + threadIdx.x;
+        __syncthreads();
+        if (j < n) { s_xy[threadIdx.x] = d.pxy[j]; s_zm[threadIdx.x] = d.pzm[j]; }
+        __syncthreads();
+        const int cnt = (int)min((int64_t)GD_KNN_TILE, n - j0);
+        for (int t = 0; t < cnt; ++t) {
+            const double2 sxy = s_xy[t], szm = s_zm[t];
+            const double dx = __dsub_rn(sxy.x, xy.x), dy = __dsub_rn(sxy.y, xy.y), dz = __dsub_rn(szm.x, zm.x);
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            if (r2 < r2k[GD_KNN_MAXK - 1] && j0 + t != i) {
+                // insert, keeping the list ascending; an equal distance goes behind the ones already there
+                double cr = r2, cm = szm.y;
+#pragma unroll
+                for (int k = 0; k < GD_KNN_MAXK; ++k) {
+                    if (cr < r2k[k]) {
+                        const double tr = r2k[k], tm = mk[k];
+                        r2k[k] = cr; mk[k] = cm;
+                        cr = tr; cm = tm;
+                    }
+                }
+            }
+        }
+    }
+    if (!live) return;
+    // the K - 1 nearest masses, nearest first; the sphere through the K-th
+    double mass = 0.0, rK2 = r2k[0];
+#pragma unroll
+    for (int k = 0; k < GD_KNN_MAXK; ++k) {
+        if (k < K - 1) mass = __dadd_rn(mass, mk[k]);
+        if (k == K - 1) rK2 = r2k[k];
+    }
+    const double r = __dsqrt_rn(rK2);
+    const double c43 = 4.0 * 3.141592653589793 / 3.0;
+    rho[i] = __ddiv_rn(mass, __dmul_rn(__dmul_rn(__dmul_rn(c43, r), r), r));
+}
+
+// x_d and r_c from rho (fixed order: a contiguous slice per thread in index order, then a binary tree) -> out[0..2] = x_d,
+// out[3] = r_c, out[4] = sum rho, out[5] = largest rho_i
+__global__ void __launch_bounds__(1024) k_diag_core(gd_dev d, int64_t n, const double *rho, double *out)
+{
+    __shared__ double s[4][1024];
+    __shared__ double s_c[3];
+    const int tid = threadIdx.x;
+    const int64_t per = (n + 1023) / 1024, b = (int64_t)tid * per, e = min(n, b + per);
+    double w0 = 0.0, wx = 0.0, wy = 0.0, wz = 0.0, wm = 0.0;
+    for (int64_t i = b; i < e; ++i) {
+        const double2 xy = d.pxy[i], zm = d.pzm[i];
+        const double r = rho[i];
+        w0 += r; wx += r * xy.x; wy += r * xy.y; wz += r * zm.x;
+        wm = fmax(wm, r);
+    }
+    s[0][tid] = w0; s[1][tid] = wx; s[2][tid] = wy; s[3][tid] = wz;
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if (tid < o) for (int k = 0; k < 4; ++k) s[k][tid] += s[k][tid + o];
+        __syncthreads();
+    }
+    if (tid == 0) {
+        s_c[0] = s[1][0] / s[0][0]; s_c[1] = s[2][0] / s[0][0]; s_c[2] = s[3][0] / s[0][0];
+        out[0] = s_c[0]; out[1] = s_c[1]; out[2] = s_c[2]; out[4] = s[0][0];
+    }
+    __syncthreads();
+    const double cx = s_c[0], cy = s_c[1], cz = s_c[2];
+    double num = 0.0, den = 0.0;
+    for (int64_t i = b; i < e; ++i) {
+        const double2 xy = d.pxy[i], zm = d.pzm[i];
+        const double r = rho[i], w = r * r;
+        const double dx = xy.x - cx, dy = xy.y - cy, dz = zm.x - cz;
+        num += w * ((dx * dx + dy * dy) + dz * dz);
+        den += w;
+    }
+    __syncthreads();
+    s[0][tid] = num; s[1][tid] = den; s[2][tid] = wm;
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if (tid < o) { s[0][tid] += s[0][tid + o]; s[1][tid] += s[1][tid + o]; s[2][tid] = fmax(s[2][tid], s[2][tid + o]); }
+        __syncthreads();
+    }
+    if (tid == 0) { out[3] = sqrt(s[0][0] / s[1][0]); out[5] = s[2][0]; }
+}
+
+// rho -> rho_dev (the caller's [n] array, or the internal scratch d.phi when NULL); out_dev[6] as k_diag_core writes it
+int gdk_core_radius(gd_ctx *c, int K, double *rho_dev, double *out_dev)
+{
+    double *rho = rho_dev ? rho_dev : c->d.phi;
+    k_diag_knn<<<(unsigned)((c->n + GD_KNN_TILE - 1) / GD_KNN_TILE), GD_KNN_TILE, 0, c->stream>>>(c->d, c->n, K, rho);
+    GD_LAUNCH_CHECK(c, "k_diag_knn");
+    k_diag_core<<<1, 1024, 0, c->stream>>>(c->d, c->n, rho, out_dev);
+    GD_LAUNCH_CHECK(c, "k_diag_core");
+    return 0;
+}

@@ -519,6 +519,52 @@ def test_lagrange_radii_follow_the_predicted_state_and_reject_bad_fractions(gd):
     h.close()
 
 
+# ------------------------------------------------------------------ time-step census, density centre, core radius
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (4, 3000), (5, 2047), (2, 257)])
+def test_level_census_matches_oracle(gd, cfg, n):
+    # P:343 / Fig. 13: particles per CURRENT block step, at t = 0 and after 60 block steps (not the steps-taken histogram)
+    from oracle import structure
+    w = W.config(cfg, n=n)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    c0 = h.level_census()
+    assert np.array_equal(c0, structure.level_census(o.dt)) and c0.sum() == w.n
+    h.step(60)
+    for _ in range(60):
+        o.step()
+    c1 = h.level_census()
+    assert np.array_equal(c1, structure.level_census(o.dt)) and c1.sum() == w.n
+    assert not np.array_equal(c1, h.level_histogram()[0])
+    h.close()
+
+
+@pytest.mark.parametrize("cfg,n,k", [(1, 1024, 6), (4, 3000, 6), (4, 700, 2), (5, 2047, 8), (2, 300, 6)])
+def test_core_radius_matches_oracle(gd, cfg, n, k):
+    # P:341 / Fig. 12, reading R25 (Casertano & Hut 1985): rho_i element by element, density centre and core radius
+    from oracle import structure
+    w = W.config(cfg, n=n)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    rc, xd, rho = h.core_radius(k, want_rho=True)
+    rc_ref, xd_ref, rho_ref = structure.core_radius(w.m, w.x, k)
+    rho = rho.cpu().numpy()
+    # every operation of rho_i is rounded as the definition writes it: the same K neighbours, the same doubles
+    assert np.abs(rho / rho_ref - 1.0).max() <= 4e-16, np.abs(rho / rho_ref - 1.0).max()
+    assert abs(rc / rc_ref - 1.0) < 1e-12 and np.abs(xd - xd_ref).max() < 1e-12 * max(1.0, np.abs(w.x).max())
+    # off a synchronisation time the predicted positions are what is looked at
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    h.step(33)
+    for _ in range(33):
+        o.step()
+    xp, _ = oracle.predict(o.t, o.x, o.v, o.a, o.j, o.t_i)
+    rc2, xd2 = h.core_radius(k)
+    rc2_ref, xd2_ref, _ = structure.core_radius(w.m, xp, k)
+    assert abs(rc2 / rc2_ref - 1.0) < 1e-10 and np.abs(xd2 - xd2_ref).max() < 1e-10
+    for bad in (1, 9):
+        with pytest.raises(gd.GravidyError):
+            h.core_radius(bad)
+    h.close()
+
+
 # ------------------------------------------------------------------------------ options that change the schedule
 @pytest.mark.parametrize("use_loop", [True, False])
 def test_single_halving_variant_matches_oracle(gd, use_loop):
