@@ -19,6 +19,10 @@ available, so the same *distributions* are sampled here from
   [0.5, 100], continuous at 0.5) by inverse CDF, normalised to total mass 1.
 
 ``config(k)`` builds the five BASELINE.json configs C1..C5.
+
+Two further workloads from the paper's list of applications (section 6: "the collision of two
+clusters", "a central massive particle"), Newtonian only (the post-Newtonian pair of PAPER.md:351-355 has no equations
+in the reference): ``two_cluster_collision`` and ``central_massive_particle``.
 """
 from __future__ import annotations
 
@@ -29,7 +33,7 @@ import numpy as np
 
 __all__ = [
     "Workload", "plummer", "kroupa_masses", "config", "active_indices",
-    "CONFIG_N", "two_body", "random_cluster",
+    "CONFIG_N", "two_body", "random_cluster", "two_cluster_collision", "central_massive_particle",
 ]
 
 #: particle counts of BASELINE.json configs C1..C5 (C5 has one extra central particle)
@@ -180,3 +184,54 @@ def random_cluster(n: int, seed: int, eps: float = 1e-4) -> Workload:
     v = (rng.random((n, 3)) * 2.0 - 1.0) * 0.5
     return Workload(f"random-{n}", m, np.ascontiguousarray(x), np.ascontiguousarray(v), eps, 0.01, 0.0,
                     {"seed": seed})
+
+
+def two_cluster_collision(n: int, seed: int, mass_ratio: float = 1.0, apocentre: float = 3.0, ecc: float = 0.5,
+                          eps: float = 1e-4, t_end: float = 0.25) -> Workload:
+    """"The collision of two clusters": two Plummer spheres with n1 : n2 = M1 : M2 = mass_ratio : 1
+    (equal particle masses, total mass 1), each sampled like C1-C3 and scaled to its own mass at unchanged length
+    scale (velocities x sqrt(M_k)), set on a bound Kepler orbit of their centres of mass: they start at the apocentre
+    distance ``apocentre`` along x, moving along +-y with the two-body apocentre speed of eccentricity ``ecc``, so that
+    point masses would pass at apocentre (1 - ecc) / (1 + ecc) -- inside each other for the defaults.  The centre of
+    mass of the whole system is at rest at the origin.  Particles 0 .. n1-1 are cluster 1."""
+    n1 = int(round(n * mass_ratio / (1.0 + mass_ratio)))
+    n1 = min(max(n1, 1), n - 1)
+    n2 = n - n1
+    mp = 1.0 / n
+    M1, M2 = n1 * mp, n2 * mp
+    _, x1, v1 = plummer(n1, seed=seed)
+    _, x2, v2 = plummer(n2, seed=seed + 1)
+    v1 = v1 * math.sqrt(M1)
+    v2 = v2 * math.sqrt(M2)
+    # relative orbit of the centres: separation d at apocentre, speed sqrt(M (1 - e) / d), G = M = 1
+    d = float(apocentre)
+    vrel = math.sqrt((M1 + M2) * (1.0 - ecc) / d)
+    x1 = x1 + np.array([-M2 * d, 0.0, 0.0])
+    x2 = x2 + np.array([M1 * d, 0.0, 0.0])
+    v1 = v1 + np.array([0.0, -M2 * vrel, 0.0])
+    v2 = v2 + np.array([0.0, M1 * vrel, 0.0])
+    m = np.full(n, mp, dtype=np.float64)
+    x = np.ascontiguousarray(np.concatenate([x1, x2]))
+    v = np.ascontiguousarray(np.concatenate([v1, v2]))
+    return Workload(f"two-clusters-{n1}+{n2}", m, x, v, eps, 0.01, t_end,
+                    {"seed": seed, "n1": n1, "n2": n2, "M1": M1, "M2": M2, "apocentre": d, "ecc": ecc, "vrel": vrel,
+                     "semi_major": d / (1.0 + ecc)})
+
+
+def central_massive_particle(n: int, seed: int, m_central: float = 0.05, eps: float = 1e-5, t_end: float = 0.125) -> Workload:
+    """"A central massive particle" with a small softening: an equal-mass Plummer sphere of n particles
+    and total mass 1 - m_central, scaled from the unit-mass sample at unchanged length scale (velocities x
+    sqrt(1 - m_central)), plus ONE particle of mass m_central (index n: m_central n / (1 - m_central) stellar masses) at
+    rest at the origin; the centre of mass of the whole system is then put at rest at the origin.  Not an equilibrium:
+    the stars inside the heavy particle's sphere of influence fall towards it, and it wanders -- it takes part in the
+    dynamics, unlike the 0.01 point mass of the throughput config C5."""
+    _, x, v = plummer(n, seed=seed)
+    ms = (1.0 - m_central) / n
+    v = v * math.sqrt(1.0 - m_central)
+    m = np.concatenate([np.full(n, ms), [m_central]])
+    x = np.concatenate([x, np.zeros((1, 3))])
+    v = np.concatenate([v, np.zeros((1, 3))])
+    x = x - (m[:, None] * x).sum(axis=0) / m.sum()
+    v = v - (m[:, None] * v).sum(axis=0) / m.sum()
+    return Workload(f"central-massive-{n}+1", np.ascontiguousarray(m), np.ascontiguousarray(x), np.ascontiguousarray(v),
+                    eps, 0.01, t_end, {"seed": seed, "m_central": m_central, "m_star": ms})

@@ -519,6 +519,48 @@ def test_lagrange_radii_follow_the_predicted_state_and_reject_bad_fractions(gd):
     h.close()
 
 
+# --------------------------------------------------- the paper's further applications, Newtonian part
+def _further_workload(kind):
+    if kind == "two_clusters":
+        return W.two_cluster_collision(3000, seed=11, mass_ratio=2.0)          # P:390 "the collision of two clusters"
+    return W.central_massive_particle(2500, seed=21, m_central=0.05)          # P:392 "a central massive particle", eps = 1e-5
+
+
+@pytest.mark.parametrize("kind", ["two_clusters", "central_massive"])
+def test_further_workloads_match_oracle(gd, kind):
+    # same bar as the five configs: a, jerk 1e-12 and dt bit-exact at init, the first 100 block steps bit-exact, the
+    # energy error at the end of a short run within 10 % of the oracle's
+    w = _further_workload(kind)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    s = h.state_host(("a", "j", "dt"))
+    assert relnorm(s["a"], o.a).max() < 1e-12 and relnorm(s["j"], o.j).max() < 1e-12 and np.array_equal(s["dt"], o.dt)
+    k0, u0 = h.energy()
+    K0, U0 = o.energy()
+    assert abs(k0 / K0 - 1) < 1e-13 and abs(u0 / U0 - 1) < 1e-13
+    for k in range(100):
+        t_next, cnt = h.next_block()
+        act = h.active().cpu().numpy()
+        o.step()
+        assert t_next == o.t and np.array_equal(act, o.active), f"schedule differs at block step {k}"
+        h.predict(t_next)
+        h.force_jerk(None)
+        h.correct_and_timestep()
+    s = h.state_host(("x", "t", "dt"))
+    assert np.array_equal(s["t"], o.t_i) and np.array_equal(s["dt"], o.dt) and np.abs(s["x"] - o.x).max() < 1e-12
+    # on through the persistent loop to the workload's end time
+    steps, psteps = h.run_until(w.t_end)
+    o.run(w.t_end)
+    assert h.block_steps == o.block_steps and h.particle_steps == o.particle_steps and h.t == o.t == w.t_end
+    k1, u1 = h.energy()
+    K1, U1 = o.energy()
+    err, err_ref = abs((k1 + u1) / (k0 + u0) - 1), abs((K1 + U1) / (K0 + U0) - 1)
+    assert err_ref < 1e-5 and abs(err / err_ref - 1.0) < 0.10, (err, err_ref)
+    s = h.state_host(("t", "dt"))
+    assert np.array_equal(s["t"], o.t_i) and np.array_equal(s["dt"], o.dt)
+    h.close()
+
+
 # ------------------------------------------------------------------ time-step census, density centre, core radius
 @pytest.mark.parametrize("cfg,n", [(1, 1024), (4, 3000), (5, 2047), (2, 257)])
 def test_level_census_matches_oracle(gd, cfg, n):

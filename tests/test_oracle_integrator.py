@@ -363,3 +363,40 @@ def test_plain_and_compensated_integrations_stay_close():
     rb = ob.run(max_steps=100, record=True)
     assert np.array_equal(ra[0], rb[0]) and np.array_equal(ra[2], rb[2])    # same schedule, bit for bit
     assert np.abs(oa.x - ob.x).max() < 1e-12
+
+
+# ------------------------------------------------------------------- further applications, Newtonian part
+def test_two_cluster_collision_dynamics():
+    # two bound Plummer spheres falling towards each other: the relative acceleration of their centres is that of point
+    # masses, -M / d^2, reduced by the part of each sphere that lies beyond the other's centre (Plummer tails: 5 % of
+    # the mass is outside r = 3)
+    w = W.two_cluster_collision(600, seed=11, mass_ratio=1.0, apocentre=3.0, ecc=0.5)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    n1 = w.meta["n1"]
+    K0, U0 = o.energy()
+    a_rel = o.a[n1:].mean(0) - o.a[:n1].mean(0)
+    assert 0.75 < a_rel[0] / (-1.0 / 9.0) < 1.0 and abs(a_rel[1]) < 0.01 and abs(a_rel[2]) < 0.01
+    o.run(0.5)
+    sep = np.linalg.norm(o.x[n1:].mean(0) - o.x[:n1].mean(0))
+    # near apocentre r(t) ~ d - (|a_rel| - vrel^2 / d) t^2 / 2 (radial acceleration minus the centrifugal term): the
+    # centres of mass move as the sums of the forces say (internal forces cancel, Eq. 1)
+    expect = 3.0 - 0.5 * (abs(a_rel[0]) - w.meta["vrel"] ** 2 / 3.0) * 0.25
+    assert abs(sep - expect) < 0.01, (sep, expect)
+    K, U = o.energy()
+    assert abs((K + U) / (K0 + U0) - 1.0) < 1e-6 and o.nan_count == 0
+
+
+def test_central_massive_particle_takes_part_in_the_dynamics():
+    w = W.central_massive_particle(500, seed=21, m_central=0.05)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta)
+    K0, U0 = o.energy()
+    # momentum: sum m a = 0 with the heavy particle included, and its own acceleration is not negligible
+    assert np.abs((w.m[:, None] * o.a).sum(0)).max() < 1e-13
+    assert np.linalg.norm(o.a[-1]) > 1e-3
+    x0 = o.x[-1].copy()
+    o.run(0.125)
+    K, U = o.energy()
+    assert abs((K + U) / (K0 + U0) - 1.0) < 1e-5 and o.nan_count == 0
+    assert np.linalg.norm(o.x[-1] - x0) > 1e-5                         # it wanders
+    # its step is among the smallest of the system (the stars bound to it force it down)
+    assert o.dt[-1] <= np.median(o.dt)

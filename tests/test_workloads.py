@@ -134,3 +134,49 @@ def test_stored_full_size_schedules_are_well_formed(cfg, n):
     assert all(1 <= s[1] <= n for s in steps)
     assert sum(s[1] for s in steps) == int(kv["particle_steps"][0]) == sum(int(c) for c in kv["level_hist"])
     assert float(kv["min_margin"][0]) > 1e-10 and int(kv["nan_count"][0]) == 0
+
+
+# ------------------------------------------------------------- the paper's further applications, Newtonian
+def test_two_cluster_collision_generator():
+    from scipy.spatial.distance import pdist
+    w = W.two_cluster_collision(3000, seed=11, mass_ratio=2.0, apocentre=3.0, ecc=0.5)
+    n1, n2 = w.meta["n1"], w.meta["n2"]
+    assert n1 == 2000 and n2 == 1000 and w.n == 3000 and abs(w.m.sum() - 1.0) < 1e-14
+    M1, M2 = w.meta["M1"], w.meta["M2"]
+    assert abs(M1 - 2.0 / 3.0) < 1e-15 and abs(M2 - 1.0 / 3.0) < 1e-15
+    # whole system: centre of mass at rest at the origin
+    assert np.abs((w.m[:, None] * w.x).sum(0)).max() < 1e-14 and np.abs((w.m[:, None] * w.v).sum(0)).max() < 1e-14
+    # the two centres: apocentre separation along x, apocentre speed of the Kepler orbit along y
+    c1, c2 = w.x[:n1].mean(0), w.x[n1:].mean(0)
+    u1, u2 = w.v[:n1].mean(0), w.v[n1:].mean(0)
+    assert np.allclose(c2 - c1, [3.0, 0, 0], atol=1e-13)
+    vrel = math.sqrt(1.0 * (1 - 0.5) / 3.0)
+    assert np.allclose(u2 - u1, [0, vrel, 0], atol=1e-13) and abs(w.meta["vrel"] - vrel) < 1e-15
+    # orbital energy and angular momentum of two point masses on that orbit: E = -M1 M2 / 2a, a = d / (1 + e)
+    mu = M1 * M2 / (M1 + M2)
+    E_orb = 0.5 * mu * vrel ** 2 - M1 * M2 / 3.0
+    assert abs(E_orb - (-M1 * M2 / (2.0 * w.meta["semi_major"]))) < 1e-15
+    # each cluster alone is a Plummer sphere of its mass in virial equilibrium: 2K/|U| = 1 in its own frame
+    for sl, M in ((slice(0, n1), M1), (slice(n1, None), M2)):
+        m, x, v = w.m[sl], w.x[sl], w.v[sl] - w.v[sl].mean(0)
+        K = 0.5 * (m * (v * v).sum(1)).sum()
+        iu = np.triu_indices(len(m), 1)
+        U = -(m[iu[0]] * m[iu[1]] / pdist(x)).sum()
+        assert abs(2 * K / abs(U) - 1.0) < 0.06
+        assert abs((K + U) / (-0.25 * M * M) - 1.0) < 0.08      # E = -M^2 / 4 at unit length scale
+    # deterministic, and a different seed differs
+    w2 = W.two_cluster_collision(3000, seed=11, mass_ratio=2.0)
+    assert np.array_equal(w.x, w2.x) and not np.array_equal(w.x, W.two_cluster_collision(3000, seed=12, mass_ratio=2.0).x)
+
+
+def test_central_massive_particle_generator():
+    w = W.central_massive_particle(2048, seed=21, m_central=0.05)
+    assert w.n == 2049 and abs(w.m.sum() - 1.0) < 1e-14 and w.m[-1] == 0.05
+    assert abs(w.m[-1] / w.m[0] - 0.05 * 2048 / 0.95) < 1e-9          # ~108 stellar masses
+    assert np.abs((w.m[:, None] * w.x).sum(0)).max() < 1e-15 and np.abs((w.m[:, None] * w.v).sum(0)).max() < 1e-15
+    # the heavy particle starts (almost) at rest at the centre: displaced only by the removal of the centre of mass
+    assert np.linalg.norm(w.x[-1]) < 1e-12 and np.linalg.norm(w.v[-1]) < 1e-12
+    assert w.eps == 1e-5 and w.eps < 1e-4                              # "small epsilon"
+    # the stars: a Plummer sphere of mass 0.95 at the unit-mass length scale (half-mass radius 0.7686)
+    r = np.sort(np.linalg.norm(w.x[:-1], axis=1))
+    assert abs(r[1024] - 0.7686) < 0.05
