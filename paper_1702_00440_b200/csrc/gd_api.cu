@@ -202,7 +202,9 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = cudaHostAlloc((void **)&c->h_cell, 64, cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->coop, cudaDevAttrCooperativeLaunch, dev);
+    if (e == cudaSuccess) e = cudaHostAlloc((void **)&c->h_cell, 64, cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer((void **)&c->h_cell_dev, c->h_cell, 0);
     if (e == cudaSuccess) e = cudaHostAlloc((void **)&c->h_ctrl, 2 * sizeof(gd_ctrl), cudaHostAllocDefault);
     if (e != cudaSuccess) {
         gd_fail_cuda(nullptr, e, "gd_init: no usable CUDA device (there is no CPU fallback)");
@@ -329,9 +331,11 @@ extern "C" int gd_next_block(gd_ctx *c, double *t_next_host, int64_t *n_act_host
 {
     if (!c) return GD_EINVAL;
     if (c->lvl_min > c->lvl_max) return gd_fail(c, GD_ESTATE, "gd_next_block: dt_level_min > dt_level_max");
-    int rc = gdk_next_block(c);
+    bool wrote_host = false;
+    int rc = gdk_next_block(c, false, c->h_cell_dev, &wrote_host);
     if (rc) return rc == GD_ECUDA ? rc : GD_EINVAL;          // text already in c->err
-    GD_CUDA(c, cudaMemcpyAsync(c->h_cell, c->d.cell, 16, cudaMemcpyDeviceToHost, c->stream));
+    // the one-kernel form writes {t_next, n_act} into the pinned words itself: no copy to enqueue
+    if (!wrote_host) GD_CUDA(c, cudaMemcpyAsync(c->h_cell, c->d.cell, 16, cudaMemcpyDeviceToHost, c->stream));
     GD_CUDA(c, cudaStreamSynchronize(c->stream));
     c->t_next = c->h_cell[0];
     long long na;

@@ -74,7 +74,9 @@ struct gd_ctx {
     int64_t jsplit_max_nact;
     cudaStream_t stream;
     gd_dev d;
-    double *h_cell;              // pinned host mirror of d.cell
+    double *h_cell;              // pinned host mirror of d.cell (mapped: h_cell_dev is its address on the device)
+    double *h_cell_dev;
+    int coop;                    // the device can launch cooperative kernels
     // host-side step state
     double t, t_next;
     int64_t n_act;
@@ -130,7 +132,7 @@ int gdk_force_dev(gd_ctx *c);
 int gdk_force_setup(gd_ctx *c);
 
 int gdk_correct(gd_ctx *c, double t_next, bool dev = false);                                 // gd_correct.cu
-int gdk_next_block(gd_ctx *c, bool dev = false);                                             // gd_next_block.cu
+int gdk_next_block(gd_ctx *c, bool dev = false, double *host_cell = nullptr, bool *wrote_host = nullptr);   // gd_next_block.cu
 int gdk_loop_setup(gd_ctx *c);                                                               // gd_loop.cu
 int gdk_loop(gd_ctx *c);
 int gdk_slice_setup(gd_ctx *c);

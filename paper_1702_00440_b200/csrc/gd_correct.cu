@@ -11,8 +11,11 @@
 #include "gd_hermite.cuh"
 
 #define GD_CB 128
+#ifndef GD_CB_MIN
+#define GD_CB_MIN 8              // resident CTAs per SM the compiler is asked to fit (register cap 65536 / (GD_CB x GD_CB_MIN))
+#endif
 
-__global__ void __launch_bounds__(GD_CB)
+__global__ void __launch_bounds__(GD_CB, GD_CB_MIN)
 k_correct_timestep(gd_dev d, int n_act, double t_next, double eta, double dt_min, double dt_max, int halving_mode, int dev)
 {
     // dev != 0 (block-step graph): the active count and t_next come from device memory, the grid is fixed and

@@ -234,8 +234,143 @@ k_block_select(gd_dev d, int64_t np, int dev)
     }
 }
 
-int gdk_next_block(gd_ctx *c, bool dev)
+// ---------------------------------------------------------------------------------------------------------
+// Mid-size systems (up to sm_count x 1024 x 16 particles: C4, C5): ONE cooperative kernel, one CTA per SM, tnext read
+// once.  Thread t of block b owns the contiguous chunk [(b 1024 + t) R, +R) and keeps it in registers:
+//   block minimum -> one 64-bit atomic per block on the grid minimum (non-negative doubles order like their bit patterns; the
+//   word holds the COMPLEMENT under atomicMax, so that its rest state is the zero the scratch is cleared to) -> grid
+//   barrier (arrival counter: the launch is cooperative, every block is resident) -> match flags from the registers ->
+//   block-wide exclusive scan -> the block's count goes to agg[b] with the epoch, the counts of the lower blocks are
+//   waited for -> ordered writes.  The last block to finish re-arms the counters.
+// The result {t_next, n_act} also goes straight to the caller's pinned host words (host_cell, mapped): gd_next_block
+// then needs one launch and one stream synchronisation, no copy.
+template <int R>
+__global__ void __launch_bounds__(GD_SCAN_THREADS, 1)
+k_block_one(gd_dev d, int64_t np, int dev, double *host_cell)
 {
+    __shared__ double s_min[32];
+    __shared__ int s_cnt[32];
+    __shared__ int s_prefix;
+    __shared__ double s_t;
+    if (dev && d.ctrl->finished) return;                         // set only behind the grid barrier below: uniform
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const unsigned int bid = blockIdx.x, G = gridDim.x;
+    const int64_t base = ((int64_t)bid * GD_SCAN_THREADS + tid) * R;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    unsigned long long *gmax = reinterpret_cast<unsigned long long *>(d.blockmin + GD_SCAN_MAX_BLOCKS - 1);
+    const unsigned int epoch = d.ticket[2] + 1u ? d.ticket[2] + 1u : 1u;     // read before the barrier, advanced behind it
+    bool stop = false;
+    if (dev) {
+        const gd_ctrl *ct = d.ctrl;
+        stop = ct->t >= ct->t_end || (ct->max_steps >= 0 && ct->steps >= ct->max_steps);
+    }
+    double v[R];
+    double m = inf;
+#pragma unroll
+    for (int k = 0; k < R; k += 2) {
+        const double2 x = (base + k < np) ? __ldcg(reinterpret_cast<const double2 *>(d.tnext + base + k)) : make_double2(inf, inf);
+        v[k] = x.x; v[k + 1] = x.y;
+        m = fmin(m, fmin(x.x, x.y));
+    }
+    m = gd_warp_min(m);
+    if (lane == 0) s_min[warp] = m;
+    __syncthreads();
+    if (warp == 0) {
+        m = gd_warp_min(s_min[lane]);
+        if (lane == 0) {
+            atomicMax(gmax, ~(unsigned long long)__double_as_longlong(m));
+            __threadfence();
+            atomicAdd(&d.ticket[0], 1u);
+            unsigned int seen;
+            do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(d.ticket) : "memory"); } while (seen < G);
+            s_t = __longlong_as_double((long long)~__ldcg(gmax));
+        }
+    }
+    __syncthreads();
+    const double t_next = s_t;
+
+    unsigned int mask = 0u;                                      // R <= 16 match flags of this thread's chunk
+#pragma unroll
+    for (int k = 0; k < R; ++k) mask |= (unsigned int)(v[k] == t_next) << k;
+    const int cnt = stop ? 0 : __popc(mask);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += u; }
+    if (lane == 31) s_cnt[warp] = incl;
+    __syncthreads();
+    int wsum = s_cnt[lane], wincl = wsum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, wincl, o); if (lane >= o) wincl += u; }
+    const int total = __shfl_sync(0xffffffffu, wincl, 31);
+    int pos = __shfl_sync(0xffffffffu, wincl - wsum, warp) + incl - cnt;     // exclusive prefix of this thread inside the block
+    if (tid == 0) atomicExch(&d.agg[bid], ((unsigned long long)epoch << 32) | (unsigned int)total);
+    if (warp == 0) {                                             // counts of the lower-numbered blocks (all resident)
+        int sum = 0;
+        for (unsigned int p = lane; p < bid; p += 32) {
+            unsigned long long a;
+            do { a = *((volatile unsigned long long *)&d.agg[p]); } while ((unsigned int)(a >> 32) != epoch);
+            sum += (int)(unsigned int)a;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        if (lane == 0) s_prefix = sum;
+    }
+    __syncthreads();
+    pos += s_prefix;
+    if (!stop) {
+        while (mask) {
+            const int k = __ffs((int)mask) - 1;
+            mask &= mask - 1;
+            d.idx[pos++] = (int32_t)(base + k);
+        }
+    }
+    if (tid == 0) {
+        if (bid == G - 1) {                                      // the highest block knows the whole count
+            if (stop) {
+                d.ctrl->finished = 1;
+                ((long long *)d.cell)[1] = 0;
+            } else {
+                const long long n_act = (long long)(s_prefix + total);
+                d.cell[0] = t_next;
+                ((long long *)d.cell)[1] = n_act;
+                if (host_cell) { host_cell[0] = t_next; ((long long *)host_cell)[1] = n_act; }
+            }
+        }
+        __threadfence();
+        if (atomicAdd(&d.ticket[1], 1u) == G - 1) {              // every block is through: re-arm for the next launch
+            d.ticket[0] = 0u;
+            d.ticket[1] = 0u;
+            d.ticket[2] = epoch;
+            *gmax = 0ull;
+        }
+    }
+}
+
+template <int R>
+static int gd_launch_block_one(gd_ctx *c, int blocks, bool dev, double *host_cell)
+{
+    int dv = dev ? 1 : 0;
+    int64_t np = c->np;
+    void *args[] = {(void *)&c->d, (void *)&np, (void *)&dv, (void *)&host_cell};
+    cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_block_one<R>, dim3((unsigned)blocks), dim3(GD_SCAN_THREADS), args, 0, c->stream);
+    if (e != cudaSuccess) return gd_fail_cuda(c, e, "k_block_one");
+    c->launches += 1;
+    return 0;
+}
+
+// host_cell: device-side address of the caller's pinned {t_next, n_act} words, or NULL (graph path; kernels that cannot write it)
+int gdk_next_block(gd_ctx *c, bool dev, double *host_cell, bool *wrote_host)
+{
+    if (wrote_host) *wrote_host = false;
+    if (c->np > 64 * GD_SCAN_THREADS && c->coop && c->np <= (int64_t)c->sm_count * GD_SCAN_THREADS * 16) {
+        const int64_t per_sm = (c->np + (int64_t)c->sm_count * GD_SCAN_THREADS - 1) / ((int64_t)c->sm_count * GD_SCAN_THREADS);
+        const int R = per_sm <= 4 ? 4 : (per_sm <= 8 ? 8 : 16);
+        const int blocks = (int)((c->np + (int64_t)GD_SCAN_THREADS * R - 1) / ((int64_t)GD_SCAN_THREADS * R));
+        if (wrote_host) *wrote_host = host_cell != nullptr;
+        if (R == 4) return gd_launch_block_one<4>(c, blocks, dev, host_cell);
+        if (R == 8) return gd_launch_block_one<8>(c, blocks, dev, host_cell);
+        return gd_launch_block_one<16>(c, blocks, dev, host_cell);
+    }
     if (c->np <= 64 * GD_SCAN_THREADS) {
         const int dv = dev ? 1 : 0;
         if (c->np <= 4 * GD_SCAN_THREADS) k_block_select<4, true><<<1, GD_SCAN_THREADS, 0, c->stream>>>(c->d, c->np, dv);
