@@ -162,6 +162,7 @@ struct gd_lsm {
     int *smap;                       // [GD_LP_MAX_SMALL] active list position -> row of `rec` (small mode)
     double2 *sink;                   // [GD_LP_MAX_SMALL][4] the sink records of the step (small mode)
     int *spre;                       // [GD_LP_MAX_GRID + 1] exclusive prefix of the contributing candidate counts
+    int *p0t;                        // [GD_LP_MAX_GRID + 1] first particle of every CTA's slice (k_block_loop fills it once)
     double *red;                     // [GD_LP_WARPS][4][6][32] warp partial sums of a split evaluation
     double *wmin;                    // [GD_LP_WARPS]
     int *wcnt;                       // [GD_LP_WARPS + 1]
@@ -172,7 +173,7 @@ struct gd_lsm {
 __host__ __device__ inline size_t gd_lsm_bytes(int S, int state)
 {
     return (size_t)S * (16 * 3 + 8 + 8 + 4 + (state ? 128 : 0)) + GD_LP_WARPS * 4 * 6 * 32 * 8 + GD_LP_WARPS * 8 + GD_LP_MAX_SMALL * (4 + 64) +
-           (GD_LP_MAX_GRID + 1) * 4 + (GD_LP_WARPS + 1) * 4 + 66 * 4 + 64;
+           2 * (GD_LP_MAX_GRID + 1) * 4 + (GD_LP_WARPS + 1) * 4 + 66 * 4 + 64;
 }
 
 __device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S, int state)
@@ -197,6 +198,7 @@ __device__ __forceinline__ gd_lsm gd_lsm_carve(unsigned char *base, int S, int s
     s.lact = (int *)p; p += (size_t)S * 4;
     s.smap = (int *)p; p += GD_LP_MAX_SMALL * 4;
     s.spre = (int *)p; p += (GD_LP_MAX_GRID + 1) * 4;
+    s.p0t = (int *)p; p += (GD_LP_MAX_GRID + 1) * 4;
     s.wcnt = (int *)p; p += (GD_LP_WARPS + 1) * 4;
     s.hist = (unsigned int *)p;
     return s;
@@ -423,7 +425,7 @@ __device__ __forceinline__ int gd_lp_row_of(const gd_lsm &sm, int pos, int n, in
         const int mid = (lo + hi) >> 1;
         if (sm.spre[mid] <= pos) lo = mid; else hi = mid;
     }
-    return gd_slice_begin(lo, n, G) + (pos - sm.spre[lo]);
+    return sm.p0t[lo] + (pos - sm.spre[lo]);
 }
 
 // sink at a position of the active list
@@ -713,6 +715,7 @@ k_block_loop(gd_dev d, gd_largs la)
         }
     }
     if (tid < 66) sm.hist[tid] = 0u;
+    if (tid <= G) sm.p0t[tid] = gd_slice_begin(tid, la.n, G);
     __syncthreads();
     double L_me;
     int cnt_me = gd_publish(d, sm, me, p0, cnt_own, &L_me);
