@@ -489,7 +489,10 @@ static int gd_graph_build(gd_ctx *c)
     cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeRelaxed);
     int rc = 0;
     if (e == cudaSuccess) {
-        for (int k = 0; k < GD_GRAPH_STEPS && !rc; ++k) {
+        // with the persistent loop in front, one iteration is a whole run of small steps plus the one step that made the loop
+        // leave: a short graph keeps the count of idle nodes behind a finished run low
+        const int reps = c->loop_grid > 0 ? GD_GRAPH_STEPS / 4 : GD_GRAPH_STEPS;
+        for (int k = 0; k < reps && !rc; ++k) {
             // the persistent loop takes every run of small steps; the stage kernels behind it take the one step
             // that made it leave (active set above loop_hi) and do nothing once the run is finished
             rc = gdk_loop(c);
