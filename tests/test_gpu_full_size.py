@@ -192,3 +192,32 @@ def test_contexts_of_different_sizes_coexist(gd):
     assert hb.loop_profile()["block_steps"] == 80 and hs.loop_profile()["block_steps"] == 40
     check_invariants(hb.state_host(("t", "dt")), hb.t)
     hb.close(); hs.close()
+
+
+@pytest.mark.parametrize("n", [70001, 600000, 1300000])
+def test_next_block_one_kernel_form_at_every_chunk_width(gd, n):
+    # gd_next_block of mid-size systems is one cooperative kernel whose threads keep 4, 8 or 16 values of t_i + dt_i in
+    # registers (65 537 .. 606 208 / .. 1 212 416 / .. 2 424 832 particles on 148 SMs): the three widths against the
+    # definition applied to the device's own (t_i, dt_i), on the first block and after some block steps, and in
+    # the all-active case (shared step)
+    w = W.config(2, n=n)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    for stage in range(3):
+        s = h.state_host(("t", "dt"))
+        t_ref, act_ref = oracle.next_block(s["t"], s["dt"])
+        t_next, n_act = h.next_block()
+        assert t_next == t_ref and n_act == len(act_ref) and np.array_equal(cpu(h.active()), act_ref)
+        h.next_block()                                       # a second call re-arms its counters correctly
+        assert np.array_equal(cpu(h.active()), act_ref)
+        if stage == 0:
+            h.step(3)
+        elif stage == 1 and n <= 600000:
+            h.step(20)                                       # through the persistent loop or the graph of stage kernels
+    h.close()
+    if n == 70001:                                           # every particle active at once: the ordered write of the whole list
+        h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+        h.set_option("dt_level_min", 9)
+        h.set_option("dt_level_max", 9)
+        t_next, n_act = h.next_block()
+        assert t_next == 2.0 ** -9 and n_act == n and np.array_equal(cpu(h.active()), np.arange(n, dtype=np.int32))
+        h.close()
