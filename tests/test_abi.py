@@ -58,6 +58,10 @@ def test_bad_arguments_are_rejected_before_any_cuda_call(binding):
     assert lib.gd_init(C.byref(h), 16, 1, 1, 1, 1e-4, 0.01, 256, 16, None) == binding.GD_EINVAL      # too small
     assert lib.gd_init(C.byref(h), 16, 1, 1, 1, 1e-4, 0.01, 264, 1 << 30, None) == binding.GD_EINVAL  # misaligned
     assert b"gd_init" in lib.gd_last_error(None)
+    # ranges: n beyond the capacity of the active-set scan (2^25); a softening so small that eps^3 underflows the self pair
+    assert lib.gd_init(C.byref(h), (1 << 25) + 1, 1, 1, 1, 1e-4, 0.01, 256, 1 << 40, None) == binding.GD_EINVAL
+    assert lib.gd_init(C.byref(h), 16, 1, 1, 1, 1e-150, 0.01, 256, 1 << 30, None) == binding.GD_EINVAL
+    assert b"eps" in lib.gd_last_error(None)
     assert lib.gd_predict(None, 0.0) == binding.GD_EINVAL
     lib.gd_destroy(None)
 

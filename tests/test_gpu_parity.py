@@ -519,6 +519,49 @@ def test_lagrange_radii_follow_the_predicted_state_and_reject_bad_fractions(gd):
     h.close()
 
 
+# ------------------------------------------------------------------------------------------- boundary behaviour
+def test_init_host_arrays_may_be_reused_at_once(gd):
+    # gd_init_host waits for its host-to-device copies (and the repacking kernel) before it returns: scribbling over the
+    # caller's arrays right after the call must not change the initial conditions the library took
+    import torch
+    w = W.config(1)
+    ref = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    m, x, v = (torch.from_numpy(u.copy()).pin_memory().numpy() for u in (w.m, w.x, w.v))
+    h = gd.Hermite(m, x, v, w.eps, w.eta, host=True)
+    m[:] = 7.0; x[:] = np.nan; v[:] = -1.0
+    a, b = h.state_host(("x", "v", "a", "j", "dt")), ref.state_host(("x", "v", "a", "j", "dt"))
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+    h.close(); ref.close()
+
+
+def test_level_options_void_the_step_in_flight(gd):
+    # changing dt_level_min / max rewrites every dt_i: an active list or force result from before is void, and while the
+    # two levels are out of order every stage call is refused
+    w = W.config(1, n=300)
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    t_next, _ = h.next_block()
+    h.predict(t_next)
+    h.force_jerk(None)
+    h.set_option("dt_level_max", 12)
+    with pytest.raises(gd.GravidyError) as e:
+        h.correct_and_timestep()
+    assert e.value.code == gd.GD_ESTATE
+    h.set_option("dt_level_min", 14)                         # min > max: transient
+    for call in (h.next_block, lambda: h.predict(0.0), lambda: h.step(1)):
+        with pytest.raises(gd.GravidyError) as e:
+            call()
+        assert e.value.code == gd.GD_ESTATE
+    h.set_option("dt_level_max", 16)
+    o = oracle.HermiteOracle(w.m, w.x, w.v, w.eps, w.eta, dt_min=2.0 ** -16, dt_max=2.0 ** -14)
+    assert np.array_equal(h.state_host(("dt",))["dt"], o.dt)
+    h.step(20)
+    for _ in range(20):
+        o.step()
+    assert h.t == o.t and np.array_equal(h.state_host(("dt",))["dt"], o.dt)
+    h.close()
+
+
 # --------------------------------------------------- the paper's further applications, Newtonian part
 def _further_workload(kind):
     if kind == "two_clusters":
