@@ -699,6 +699,7 @@ k_block_loop(gd_dev d, gd_largs la)
     const long long ct_steps0 = steps;
     unsigned long long *bar = d.lp_ctl;
     unsigned long long target = d.lp_ctl[1];
+    unsigned long long *bar2 = d.lp_ctl + 15, target2 = d.lp_ctl[13];   // second hand-off: only the owners of a step arrive
     double *out = d.partial + (size_t)me * 6;
     const int rs = 6 * G;
     const int r0_tid = gd_slice_begin(tid < G ? tid : 0, la.n, G);   // first row of the segment of CTA `tid` (a 64-bit division: once)
@@ -747,7 +748,7 @@ k_block_loop(gd_dev d, gd_largs la)
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(GD_FULL, incl, o); if (lane >= o) incl += u; }
         if (lane == 31) sm.wcnt[warp] = incl;
-        __syncthreads();
+        const int n_con = __syncthreads_count(mine > 0);     // CTAs that contribute active particles: the owners of this step
         int wbase = 0, n_act = 0;
 #pragma unroll
         for (int w = 0; w < GD_LP_WARPS; ++w) { int c = sm.wcnt[w]; wbase += (w < warp) ? c : 0; n_act += c; }
@@ -797,10 +798,11 @@ k_block_loop(gd_dev d, gd_largs la)
         else gd_lp_force_big<EPS0>(d, sm, la, out, rs, G, n_act, cnt_own);
         GD_STAMP(3);
         g1 = gd_gtime(); const unsigned long long d0 = g1 - g0; tr[0] += d0; g0 = g1;
+        // first hand-off (all -> owners): every CTA arrives, only the owners of the step have something to wait for
         gd_bar_arrive(bar);
         GD_STAMP(4);
         target += G;
-        gd_bar_wait(bar, target);
+        if ((L_me == t_next) && cnt_me > 0) gd_bar_wait(bar, target);
         GD_STAMP(5);
         g1 = gd_gtime(); const unsigned long long d1 = g1 - g0; tr[1] += d1; g0 = g1;
         // ---- [correct] + [publish] ----
@@ -829,10 +831,12 @@ k_block_loop(gd_dev d, gd_largs la)
         psteps += n_act;
         g1 = gd_gtime(); const unsigned long long d2 = g1 - g0; tr[2] += d2; g0 = g1;
         GD_STAMP(8);
-        gd_bar_arrive(bar);
+        // second hand-off (owners -> all): only the owners arrive, everybody waits for as many arrivals as the step had
+        // owners.  (No CTA is still reading what an owner overwrites: the owner waited for every CTA's first arrival.)
+        if (contributing) gd_bar_arrive(bar2);
         GD_STAMP(9);
-        target += G;
-        gd_bar_wait(bar, target);
+        target2 += (unsigned long long)n_con;
+        gd_bar_wait(bar2, target2);
         GD_STAMP(10);
 #if GD_LP_FINE
         if (tid == 0 && fine_on) fine[14] += 1;
@@ -859,6 +863,7 @@ k_block_loop(gd_dev d, gd_largs la)
         ct->psteps += psteps;
         if (fin) ct->finished = 1;
         d.lp_ctl[1] = target;
+        d.lp_ctl[13] = target2;
         // profiling counters: particle steps and block steps taken inside the loop, ns inside it, ns per phase
         d.lp_ctl[2] += (unsigned long long)psteps;
         d.lp_ctl[3] += (unsigned long long)(steps - ct_steps0);
