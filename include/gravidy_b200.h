@@ -143,6 +143,31 @@ GD_API int gd_correct_and_timestep(gd_ctx *ctx);
  * is synchronised).  Overwrites the predicted records.  Synchronises. */
 GD_API int gd_energy(gd_ctx *ctx, double *kinetic_host, double *potential_host);
 
+/* gd_energy for callers that cannot allocate device memory -- Eq. 2, with the softened potential of gd_energy:
+ *   out_dev[0] = K = 1/2 sum m_i |v_i|^2 ;  out_dev[1] = U = - sum_{i<j} m_i m_j / sqrt(|r_ij|^2 + eps^2)
+ * of the n particles m_dev [n], x_dev [n,3], v_dev [n,3] exactly as given (no ctx, no prediction).
+ * Why it exists: all other calls need a workspace the caller obtained from cudaMalloc, and gd_init pins host memory.
+ * A program that gave all free HBM to its own pool at start-up (a later cudaMalloc fails), a loop that must not
+ * stall (cudaMalloc / cudaFree make the whole device wait), or a plug-in whose host application forbids driver
+ * allocations after start-up cannot satisfy that.  This call allocates nothing, on the device or the host: its scratch
+ * (one {K, U} pair per 256 particles) is a fixed array inside the library's device image, 128 KiB on every GPU that
+ * loads the library, held until the process exits.
+ *   - Limit: 1 <= n <= GD_ENERGY_STATIC_MAX_N; anything larger returns GD_EINVAL (nothing is truncated).
+ *   - Pointers: m_dev, x_dev, v_dev, out_dev (two doubles) are DEVICE pointers owned by the caller, on the GPU that is
+ *     current in the calling thread; cuda_stream (cudaStream_t as void*, NULL = legacy default stream) belongs to it too.
+ *   - Asynchronous: two kernels are enqueued on cuda_stream, nothing is synchronised; read out_dev in stream order.
+ *   - First call on each GPU: looks up the device address of the built-in array (and may make the CUDA runtime load
+ *     the library's device code).  Make that first call outside any stream capture.
+ *   - The array is shared by every call on that GPU and keeps the last call's contents.  No slot has to start at zero
+ *     (a call reads only what it wrote itself), and calls in one stream are ordered and safe; calls that may run
+ *     CONCURRENTLY on one GPU (different streams without an event between them) race on it -- serialise them.
+ *   - Errors: GD_EINVAL (n out of range, NULL pointer, eps negative or not finite: checked before any CUDA call),
+ *     GD_ECUDA; text from gd_energy_static_last_error() (per calling thread; never NULL). */
+#define GD_ENERGY_STATIC_MAX_N 2097152   /* 2^21 particles */
+GD_API int gd_energy_static(int64_t n, const double *m_dev, const double *x_dev, const double *v_dev, double eps,
+                            double *out_dev, void *cuda_stream);
+GD_API const char *gd_energy_static_last_error(void);
+
 /* Convenience: n_steps block steps (next_block, predict, force_jerk, correct) / block steps until t >= t_end.
  * Optional outputs (NULL to skip): steps taken, sum of active counts (particle steps).  Synchronises. */
 GD_API int gd_step(gd_ctx *ctx, int64_t n_steps, int64_t *particle_steps_host);

@@ -34,6 +34,8 @@ SYMBOLS = {
     "gd_force_jerk_host": (_int, [_i64, _vp, _vp, _vp, _dbl, _vp, _i64, _vp, _vp, _vp, _sz, _vp]),
     "gd_correct_and_timestep": (_int, [_vp]),
     "gd_energy": (_int, [_vp, _pdbl, _pdbl]),
+    "gd_energy_static": (_int, [_i64, _vp, _vp, _vp, _dbl, _vp, _vp]),
+    "gd_energy_static_last_error": (C.c_char_p, []),
     "gd_step": (_int, [_vp, _i64, _pi64]),
     "gd_run_until": (_int, [_vp, _dbl, _i64, _pi64, _pi64]),
     "gd_time": (_dbl, [_vp]),
@@ -107,6 +109,31 @@ def selftest_div_const(n: int = 1 << 24, seed: int = 1) -> int:
     if rc:
         raise GravidyError(rc, "gd_selftest_div_const failed (no CUDA device?)")
     return int(bad.value)
+
+
+#: largest n gd_energy_static accepts (GD_ENERGY_STATIC_MAX_N of the header)
+ENERGY_STATIC_MAX_N = 1 << 21
+
+
+def energy_static(m, x, v, eps: float, out, stream=None):
+    """gd_energy_static: K and U (Eq. 2) of the particles m [n], x [n,3], v [n,3] into out[0], out[1].
+
+    This is the call for code that may not allocate on the GPU -- a driver whose pool already owns all of HBM, a loop
+    that cannot afford the device-wide wait of cudaMalloc, a plug-in whose host forbids allocations -- so the wrapper
+    allocates nothing either: m, x, v and out (two doubles) must already be contiguous float64 CUDA tensors.  The
+    reduction's scratch lives in a fixed array inside the library, hence n <= ENERGY_STATIC_MAX_N and the rule that
+    two calls must not run concurrently on one GPU (calls on one stream are fine).  Asynchronous on `stream` (default:
+    torch's current stream); returns `out`.  The first call per GPU should happen outside stream capture."""
+    torch = _torch()
+    n = int(m.shape[0])
+    for t, shape in ((m, (n,)), (x, (n, 3)), (v, (n, 3)), (out, (2,))):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == shape, \
+            "energy_static takes contiguous float64 CUDA tensors m [n], x [n,3], v [n,3], out [2] and converts nothing"
+    sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+    rc = load().gd_energy_static(n, m.data_ptr(), x.data_ptr(), v.data_ptr(), float(eps), out.data_ptr(), sp)
+    if rc:
+        raise GravidyError(rc, load().gd_energy_static_last_error().decode())
+    return out
 
 
 def _torch():
