@@ -85,19 +85,29 @@ GD_API void gd_destroy(gd_ctx *ctx);
 /* Text of the last error recorded on ctx (ctx == NULL: last error of a failed gd_init). Never NULL. */
 GD_API const char *gd_last_error(const gd_ctx *ctx);
 
-/* Tunables.  key: "jsplit_max_nact" (active sets of at most this size use the j-split kernel; default 512, capped
- * at 32 x the number of clusters in its grid), "ipar_small_max_nact" (above that and up to this size the i-parallel
- * kernel runs with 32-sink tiles, beyond it with 256-sink tiles; default 2048),
+/* Tunables.  Which kernel gd_force_jerk (and the force stage of gd_step behind the persistent loop) launches is
+ * decided by the size of the active set, first match wins:
+ *   n_act <= "slice_max_nact" (default 8192; 0 = off)   k_force_slice: one CTA per SM over a shared-memory slice of
+ *                                                        the sources, every sink against it, partial rows folded per sink
+ *   n_act <= "jsplit_max_nact" (default 512, capped at 32 x the clusters of its grid)
+ *                                                        k_force_jsplit: clusters of 8 CTAs split the sources, DSMEM fold
+ *   n_act <= "ipar_small_max_nact" (default 2048)        k_force_ipar<1,4>: i-parallel, 32-sink tiles, sources split
+ *   larger                                               k_force_ipar<2,1>: i-parallel, 256-sink tiles (the all-active kernel)
+ * With the defaults the second and third rows are never reached (the slice kernel measured faster over their whole
+ * range); they run only when "slice_max_nact" is lowered, which the parity tests do.
+ * Other keys: "slice_passes" (slices per CTA of k_force_slice: 0 = the fewest whose records fit in shared memory
+ * [default: 1 up to N ~ 3.5e5, 3 at C5's size], 1..16 forces a count),
  * "dt_level_min", "dt_level_max" (override GD_LEVEL_MIN/MAX before the first step; 0 <= min <= max <= 52),
  * "halving_mode" (1: halve until dt <= dt_req [default]; 0: a single halving per step),
- * "slice_max_nact" (active sets up to this size go to k_force_slice, one CTA per SM over a shared-memory slice of
- * the sources; default 8192, 0 = off: the kernels above take over), "slice_passes" (slices per CTA of that kernel:
- * 0 = the fewest whose records fit in shared memory [default: 1 up to N ~ 3.5e5, 3 at C5's size], 1..16 forces a count),
  * "loop_max_nact", "loop_small_nact", "loop_state_smem", "loop_warp_correct" (the persistent block-step loop behind
  * gd_step / gd_run_until: largest active set it takes [default: all], size up to which lanes stride over sources
  * [96], own state resident in shared memory [1], number of own active particles up to which a CTA corrects them a
  * warp each instead of a thread each [48]),
- * "profile" (0/1: time every force launch with CUDA events, see gd_get_profile).  GD_EINVAL on unknown keys. */
+ * "loop_timers" (0/1, default 0: launch the loop's instantiation whose CTA 0 reads the device timer around every phase
+ * and fills the bins of gd_get_loop_histogram; costs about 1 % on runs of small block steps),
+ * "use_graph" (0/1, default 1: gd_step / gd_run_until replay a captured graph),
+ * "profile" (0/1: time every force launch with CUDA events, see gd_get_profile).
+ * GD_EINVAL on unknown keys. */
 GD_API int gd_set_option(gd_ctx *ctx, const char *key, double value);
 
 /* Step (v).  t_next = min_i (t_i + dt_i); the active list becomes { i ascending : t_i + dt_i == t_next }
@@ -118,7 +128,8 @@ GD_API int gd_predict(gd_ctx *ctx, double t);
  * of the last gd_next_block (then n_act is ignored).  a_out_dev / j_out_dev: [n_act,3] device arrays, or NULL
  * to keep the results in the internal buffers that gd_correct_and_timestep consumes.  With an explicit
  * idx_dev the call does not touch integrator state.  Indices are not range-checked.  n_act == 0 is a no-op.
- * Large lists use the i-parallel kernel, small lists the j-split kernel (see "jsplit_max_nact"). */
+ * The kernel is chosen by n_act as the table at gd_set_option says (by default: the source-slice kernel up to 8192
+ * sinks, the i-parallel kernel with 256-sink tiles above). */
 GD_API int gd_force_jerk(gd_ctx *ctx, const int32_t *idx_dev, int64_t n_act, double *a_out_dev, double *j_out_dev);
 
 /* One-shot form of gd_force_jerk on HOST arrays: x, v are taken as the (already predicted) state of n sources,
@@ -221,12 +232,14 @@ GD_API int gd_core_radius(gd_ctx *ctx, int k_neighbours, double *core_radius_hos
  * block steps) since init -> out_host[11] = { particle steps, block steps taken inside
  * the loop, ns spent inside it (device global timer, CTA 0), ns in its force phase, in the barrier after it, in its
  * corrector phase, in the barrier after it, launches that did work, and for CTA 0 as an owner of active particles:
- * steps, ns summing partials + correcting, ns publishing } (11 values).  Synchronises. */
+ * steps, ns summing partials + correcting, ns publishing } (11 values).  The step counts are always kept; the ns
+ * values only grow while the "loop_timers" option is on.  Synchronises. */
 GD_API int gd_get_loop_profile(gd_ctx *ctx, int64_t *out_host);
 /* The same loop's block steps binned by the size of their active set ("N_act << N": where the step count and the
  * time of a block-step run go) -> out_host[32][6]: bucket b holds the steps with bit_length(n_act) == b, i.e.
  * 2^(b-1) <= n_act < 2^b, as { block steps, particle steps, ns in the force phase, ns in the barrier after it, ns in
- * the corrector phase, ns in the barrier after it } (device global timer, CTA 0's view), since init.  Synchronises. */
+ * the corrector phase, ns in the barrier after it } (device global timer, CTA 0's view), since init; only the steps
+ * taken while the "loop_timers" option was on are binned.  Synchronises. */
 GD_API int gd_get_loop_histogram(gd_ctx *ctx, int64_t *out_host);
 
 /* Optional CUDA-event timing of the force launches, switched on with gd_set_option(ctx, "profile", 1): every

@@ -124,7 +124,7 @@ static size_t gd_carve(gd_dev *d, void *base, int64_t np, int64_t pcap)
     t.geom_l = w.take<int2>(np / 256 + 2);
     t.lp_L = w.take<double>(256);
     t.lp_cnt = w.take<int>(256);
-    t.lp_ctl = w.take<unsigned long long>(16);
+    t.lp_ctl = w.take<unsigned long long>(GD_LP_CTL_WORDS);
     t.lp_prof = w.take<unsigned long long>(GD_LP_PROF_BUCKETS * 6);
     t.diag_scratch = w.take<unsigned long long>(4352);
     t.cell = w.take<double>(4);
@@ -194,6 +194,7 @@ static int gd_create(gd_ctx **out, int64_t n, double eps, double eta, void *ws, 
     c->loop_max_nact = GD_LP_MAX_HI;          // every step the scratch allows (larger active sets: i-parallel stage kernel)
     c->loop_small_nact = 96;
     c->loop_warp_correct = 48;
+    c->loop_timers = 0;
     c->slice_max_nact = 8192;
     c->slice_passes_opt = 0;
     c->loop_state_opt = 1;
@@ -298,6 +299,7 @@ extern "C" int gd_set_option(gd_ctx *c, const char *key, double value)
         gd_graph_drop(c);
         return gdk_loop_setup(c);
     }
+    if (!strcmp(key, "loop_timers")) { c->loop_timers = value != 0.0; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "loop_warp_correct")) { c->loop_warp_correct = (int64_t)value; gd_graph_drop(c); return GD_OK; }
     if (!strcmp(key, "profile")) {
         int rc = gd_prof_drain(c);
@@ -556,7 +558,7 @@ static int gd_run_profiled(gd_ctx *c, double t_end, int64_t max_steps, int64_t *
     up->steps = up->psteps = up->finished = 0;
     unsigned long long lp0 = 0, lp1 = 0;
     GD_CUDA(c, cudaMemcpyAsync(c->d.ctrl, up, sizeof(gd_ctrl), cudaMemcpyHostToDevice, c->stream));
-    GD_CUDA(c, cudaMemcpyAsync(&lp0, c->d.lp_ctl + 2, 8, cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaMemcpyAsync(&lp0, c->d.lp_ctl + GD_LP_CTL_BASE + 2, 8, cudaMemcpyDeviceToHost, c->stream));
     for (;;) {
         const int slot = gd_prof_begin(c);
         int rc = gdk_loop(c);
@@ -570,7 +572,7 @@ static int gd_run_profiled(gd_ctx *c, double t_end, int64_t max_steps, int64_t *
         GD_CUDA(c, cudaStreamSynchronize(c->stream));
         if (down->finished) break;
     }
-    GD_CUDA(c, cudaMemcpyAsync(&lp1, c->d.lp_ctl + 2, 8, cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaMemcpyAsync(&lp1, c->d.lp_ctl + GD_LP_CTL_BASE + 2, 8, cudaMemcpyDeviceToHost, c->stream));
     GD_CUDA(c, cudaStreamSynchronize(c->stream));
     c->prof[4 * 3 + 2] += (double)(lp1 - lp0) * (double)c->n;         // pairs evaluated inside the loop
     c->t = down->t;
@@ -701,7 +703,7 @@ extern "C" int gd_get_profile(gd_ctx *c, double *prof_host)
 extern "C" int gd_get_loop_profile(gd_ctx *c, int64_t *out_host)
 {
     if (!c || !out_host) return GD_EINVAL;
-    GD_CUDA(c, cudaMemcpyAsync(out_host, c->d.lp_ctl + 2, 11 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    GD_CUDA(c, cudaMemcpyAsync(out_host, c->d.lp_ctl + GD_LP_CTL_BASE + 2, 11 * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
     GD_CUDA(c, cudaStreamSynchronize(c->stream));
     return GD_OK;
 }

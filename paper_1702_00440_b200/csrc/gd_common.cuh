@@ -51,12 +51,24 @@ struct gd_dev {
     double4 *lp_rec;             // [np + GD_LP_REC_SLACK][2] candidate records, one segment of S rows per CTA
     double *lp_L;                // [256] smallest t_i + dt_i of every CTA's slice
     int *lp_cnt;                 // [256] candidates per CTA
-    unsigned long long *lp_ctl;  // [16] {barrier arrivals, arrivals at the start of the current launch, then profiling counters:
-                                 //  particle steps, block steps, ns in the loop, ns per phase x 4, launches that ran}
+    unsigned long long *lp_ctl;  // [GD_LP_CTL_WORDS] hand-off counters and run counters of k_block_loop, three 128-byte lines:
+                                 //  word GD_LP_CTL_BAR   arrivals at the first hand-off (every CTA, once per block step; monotonic)
+                                 //  word GD_LP_CTL_BAR2  arrivals at the second hand-off (the owners of a step; monotonic)
+                                 //  words GD_LP_CTL_BASE + k, written by CTA 0 when a launch ends and read when the next begins:
+                                 //   k = 1 first hand-off's count at the start of the next launch, 13 the second's;
+                                 //   k = 2 particle steps, 3 block steps inside the loop (always kept);
+                                 //   k = 4 ns in the loop, 5..8 ns per phase, 9 launches that ran, 10..12 CTA 0 as an owner
+                                 //   (steps, ns correcting, ns publishing) -- the ns words stay 0 unless the timers are on.
+                                 //  The two polled counters have a line each so that the spinning loads of one hand-off do not
+                                 //  share a line with the arrivals of the other; anything new goes behind GD_LP_CTL_BASE + 13.
     unsigned long long *lp_prof; // [GD_LP_PROF_BUCKETS][6] per bucket b = bit length of n_act: {block steps, particle steps,
                                  //  ns in [force], in the barrier after it, in [correct], in the barrier after it} (CTA 0's view)
 };
 #define GD_LP_PROF_BUCKETS 32
+#define GD_LP_CTL_BAR 0
+#define GD_LP_CTL_BAR2 16
+#define GD_LP_CTL_BASE 32
+#define GD_LP_CTL_WORDS 48
 #ifndef GD_LP_FINE
 #define GD_LP_FINE 0               // 1: debug build with fine-grained phase stamps of the loop (gd_loop.cu)
 #endif
@@ -95,6 +107,7 @@ struct gd_ctx {
     int loop_state_opt;                  // option: keep the own state resident in shared memory when it fits
     int64_t loop_warp_correct;           // option: a CTA owning up to this many active particles corrects them a warp each
     int64_t loop_small_nact;             // option: active sets up to this size use the lanes-over-sources mapping
+    int loop_timers;                     // option: CTA 0 of k_block_loop reads the device timer per phase and fills the per-size bins
     int loop_grid, loop_S, loop_hi, loop_cap, loop_state;   // geometry of k_block_loop (loop_grid = 0: not usable)
     size_t loop_smem;
     int64_t slice_max_nact;              // option: largest active set gd_force_jerk gives to k_force_slice (0 = off)

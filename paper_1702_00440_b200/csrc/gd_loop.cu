@@ -34,8 +34,9 @@
 #endif
 #define GD_LP_WARPS (GD_LP_THREADS / 32)
 #ifndef GD_LP_PROFILE
-#define GD_LP_PROFILE 1            // 0: no device-timer reads inside the loop (gd_get_loop_profile / _histogram then report 0 ns)
-#endif
+#define GD_LP_PROFILE 1            // 1: k_block_loop also exists as an instantiation with timers, launched when the "loop_timers"
+#endif                             //    option is set (the default instantiation has none); 0: no timers at all (the ns of
+                                   //    gd_get_loop_profile / gd_get_loop_histogram stay 0)
 #ifndef GD_LP_ITEM_UNROLL
 #define GD_LP_ITEM_UNROLL 2        // unrolling of the round loop of a lanes-over-sources item
 #endif
@@ -45,6 +46,10 @@
 #define GD_LP_PRAGMA_(x) _Pragma(#x)
 #define GD_LP_PRAGMA_UNROLL(n) GD_LP_PRAGMA_(unroll n)
 #define GD_LP_MAX_GRID 256          // CTAs (one per SM); bounds the shared tables
+// Thread `tid` of every CTA handles CTA `tid`'s published minimum and candidate count, and the step's owners are counted
+// with one __syncthreads_count over those threads: every tid < G has to exist.
+static_assert(GD_LP_THREADS >= GD_LP_MAX_GRID, "k_block_loop reads one CTA's {L, count} per thread: GD_LP_THREADS must cover GD_LP_MAX_GRID");
+static_assert(GD_LP_THREADS % 32 == 0 && GD_LP_THREADS <= 1024, "GD_LP_THREADS: a multiple of 32, at most 1024");
 #define GD_LP_MAX_SMALL 256         // largest active set of the lanes-over-sources mapping (bounds the position map)
 
 struct gd_largs {
@@ -87,12 +92,13 @@ __device__ __forceinline__ void gd_bar_wait(unsigned long long *bar, unsigned lo
     __syncthreads();
 }
 
-// device global timer, read by thread 0 of CTA 0 only (the read is slow); 0 elsewhere
+// device global timer, read by thread 0 of CTA 0 of the instantiation with timers only (the read is slow); 0 elsewhere
+template <bool TIMERS>
 __device__ __forceinline__ unsigned long long gd_gtime()
 {
     unsigned long long t = 0;
 #if GD_LP_PROFILE
-    if (blockIdx.x == 0 && threadIdx.x == 0) asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    if (TIMERS && blockIdx.x == 0 && threadIdx.x == 0) asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
 #endif
     return t;
 }
@@ -677,9 +683,12 @@ __device__ __forceinline__ void gd_lp_correct_thread(const gd_dev &d, const gd_l
 }
 
 // ---------------------------------------------------------------------------------------------------------------------------
-// lp_ctl[0] = barrier arrivals (monotonic over the life of the context), lp_ctl[1] = arrivals when this launch began,
-// lp_ctl[2..9] = profiling counters (gd_get_loop_profile).
-template <bool EPS0>
+// lp_ctl (layout in gd_common.cuh): word GD_LP_CTL_BAR = arrivals at the first hand-off, word GD_LP_CTL_BAR2 = arrivals at
+// the second (both monotonic over the life of the context, a 128-byte line each), words GD_LP_CTL_BASE + 1 / + 13 = their
+// counts when this launch began, words GD_LP_CTL_BASE + 2 .. + 12 = the counters of gd_get_loop_profile.
+// TIMERS: CTA 0 reads %globaltimer around every phase and adds the step to the per-size bins of gd_get_loop_histogram
+// (six atomics per block step); without, the loop has no timer reads and no atomics besides the two hand-offs.
+template <bool EPS0, bool TIMERS>
 __global__ void __launch_bounds__(GD_LP_THREADS, 1)
 k_block_loop(gd_dev d, gd_largs la)
 {
@@ -697,9 +706,9 @@ k_block_loop(gd_dev d, gd_largs la)
     double t_cur = ct->t;
     long long steps = ct->steps, psteps = 0;
     const long long ct_steps0 = steps;
-    unsigned long long *bar = d.lp_ctl;
-    unsigned long long target = d.lp_ctl[1];
-    unsigned long long *bar2 = d.lp_ctl + 15, target2 = d.lp_ctl[13];   // second hand-off: only the owners of a step arrive
+    unsigned long long *bar = d.lp_ctl + GD_LP_CTL_BAR;
+    unsigned long long target = d.lp_ctl[GD_LP_CTL_BASE + 1];
+    unsigned long long *bar2 = d.lp_ctl + GD_LP_CTL_BAR2, target2 = d.lp_ctl[GD_LP_CTL_BASE + 13];   // second hand-off: only the owners of a step arrive
     double *out = d.partial + (size_t)me * 6;
     const int rs = 6 * G;
     const int r0_tid = gd_slice_begin(tid < G ? tid : 0, la.n, G);   // first row of the segment of CTA `tid` (a 64-bit division: once)
@@ -716,7 +725,7 @@ k_block_loop(gd_dev d, gd_largs la)
         }
     }
     if (tid < 66) sm.hist[tid] = 0u;
-    if (tid <= G) sm.p0t[tid] = gd_slice_begin(tid, la.n, G);
+    for (int k = tid; k <= G; k += GD_LP_THREADS) sm.p0t[k] = gd_slice_begin(k, la.n, G);   // G + 1 entries: G may equal GD_LP_THREADS
     __syncthreads();
     double L_me;
     int cnt_me = gd_publish(d, sm, me, p0, cnt_own, &L_me);
@@ -725,7 +734,7 @@ k_block_loop(gd_dev d, gd_largs la)
     gd_bar_wait(bar, target);
 
     bool fin = false;
-    unsigned long long tr[4] = {0, 0, 0, 0}, own[3] = {0, 0, 0}, g0 = gd_gtime(), g1;   // CTA 0's view: ns in [force], barrier, [correct], barrier
+    unsigned long long tr[4] = {0, 0, 0, 0}, own[3] = {0, 0, 0}, g0 = gd_gtime<TIMERS>(), g1;   // CTA 0's view: ns in [force], barrier, [correct], barrier
     const unsigned long long g_begin = g0;
 #if GD_LP_FINE
     long long fine[16] = {0}, fine_last = clock64();
@@ -748,7 +757,10 @@ k_block_loop(gd_dev d, gd_largs la)
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(GD_FULL, incl, o); if (lane >= o) incl += u; }
         if (lane == 31) sm.wcnt[warp] = incl;
-        const int n_con = __syncthreads_count(mine > 0);     // CTAs that contribute active particles: the owners of this step
+        // n_con = CTAs that contribute active particles = the owners of this step.  It must equal the number of CTAs whose
+        // `contributing` below is true (they are the arrivals the second hand-off waits for): CTA c publishes lp_cnt[c] > 0
+        // exactly when it has candidates at its own minimum L, so (Lc == t_next && cc > 0) here is (L_me == t_next && cnt_me > 0) there.
+        const int n_con = __syncthreads_count(mine > 0);
         int wbase = 0, n_act = 0;
 #pragma unroll
         for (int w = 0; w < GD_LP_WARPS; ++w) { int c = sm.wcnt[w]; wbase += (w < warp) ? c : 0; n_act += c; }
@@ -797,18 +809,18 @@ k_block_loop(gd_dev d, gd_largs la)
         if (small) gd_lp_force_small<EPS0>(d, sm, la, out, rs, n_act, rounds);
         else gd_lp_force_big<EPS0>(d, sm, la, out, rs, G, n_act, cnt_own);
         GD_STAMP(3);
-        g1 = gd_gtime(); const unsigned long long d0 = g1 - g0; tr[0] += d0; g0 = g1;
+        g1 = gd_gtime<TIMERS>(); const unsigned long long d0 = g1 - g0; tr[0] += d0; g0 = g1;
         // first hand-off (all -> owners): every CTA arrives, only the owners of the step have something to wait for
         gd_bar_arrive(bar);
         GD_STAMP(4);
         target += G;
         if ((L_me == t_next) && cnt_me > 0) gd_bar_wait(bar, target);
         GD_STAMP(5);
-        g1 = gd_gtime(); const unsigned long long d1 = g1 - g0; tr[1] += d1; g0 = g1;
+        g1 = gd_gtime<TIMERS>(); const unsigned long long d1 = g1 - g0; tr[1] += d1; g0 = g1;
         // ---- [correct] + [publish] ----
         const bool contributing = (L_me == t_next) && cnt_me > 0;
         if (contributing) {
-            const unsigned long long o0 = gd_gtime();
+            const unsigned long long o0 = gd_gtime<TIMERS>();
             const int pre = sm.spre[me];
             // few own active particles: a warp each (lanes over the CTAs' partial sums); many: a thread each
             if (cnt_me <= la.wc_hi) {
@@ -818,18 +830,18 @@ k_block_loop(gd_dev d, gd_largs la)
             }
             __syncthreads();
             GD_STAMP(6);
-            const unsigned long long o1 = gd_gtime();
+            const unsigned long long o1 = gd_gtime<TIMERS>();
             cnt_me = gd_publish(d, sm, me, p0, cnt_own, &L_me);
             GD_STAMP(7);
 #if GD_LP_FINE
             if (tid == 0 && fine_on) fine[15] += 1;
 #endif
-            own[0] += 1; own[1] += o1 - o0; own[2] += gd_gtime() - o1;
+            own[0] += 1; own[1] += o1 - o0; own[2] += gd_gtime<TIMERS>() - o1;
         }
         t_cur = t_next;
         steps += 1;
         psteps += n_act;
-        g1 = gd_gtime(); const unsigned long long d2 = g1 - g0; tr[2] += d2; g0 = g1;
+        g1 = gd_gtime<TIMERS>(); const unsigned long long d2 = g1 - g0; tr[2] += d2; g0 = g1;
         GD_STAMP(8);
         // second hand-off (owners -> all): only the owners arrive, everybody waits for as many arrivals as the step had
         // owners.  (No CTA is still reading what an owner overwrites: the owner waited for every CTA's first arrival.)
@@ -841,9 +853,9 @@ k_block_loop(gd_dev d, gd_largs la)
 #if GD_LP_FINE
         if (tid == 0 && fine_on) fine[14] += 1;
 #endif
-        g1 = gd_gtime(); const unsigned long long d3 = g1 - g0; tr[3] += d3; g0 = g1;
+        g1 = gd_gtime<TIMERS>(); const unsigned long long d3 = g1 - g0; tr[3] += d3; g0 = g1;
 #if GD_LP_PROFILE
-        if (me == 0 && tid == 0) {                           // per-size bins of gd_get_loop_histogram (fire-and-forget REDs)
+        if (TIMERS && me == 0 && tid == 0) {                            // per-size bins of gd_get_loop_histogram (fire-and-forget REDs)
             unsigned long long *hb = d.lp_prof + 6 * (32 - __clz(n_act));
             atomicAdd(hb, 1ull); atomicAdd(hb + 1, (unsigned long long)n_act);
             atomicAdd(hb + 2, d0); atomicAdd(hb + 3, d1); atomicAdd(hb + 4, d2); atomicAdd(hb + 5, d3);
@@ -858,19 +870,20 @@ k_block_loop(gd_dev d, gd_largs la)
     if (tid < 64 && sm.hist[tid]) atomicAdd((unsigned long long *)&d.hist[tid], (unsigned long long)sm.hist[tid]);
     if (tid < 2 && sm.hist[64 + tid]) atomicAdd((unsigned long long *)&d.diag[tid], (unsigned long long)sm.hist[64 + tid]);
     if (me == 0 && tid == 0) {
+        unsigned long long *const ctl = d.lp_ctl + GD_LP_CTL_BASE;
         ct->t = t_cur;
         ct->steps = steps;
         ct->psteps += psteps;
         if (fin) ct->finished = 1;
-        d.lp_ctl[1] = target;
-        d.lp_ctl[13] = target2;
+        ctl[1] = target;
+        ctl[13] = target2;
         // profiling counters: particle steps and block steps taken inside the loop, ns inside it, ns per phase
-        d.lp_ctl[2] += (unsigned long long)psteps;
-        d.lp_ctl[3] += (unsigned long long)(steps - ct_steps0);
-        d.lp_ctl[4] += gd_gtime() - g_begin;
-        for (int k = 0; k < 4; ++k) d.lp_ctl[5 + k] += tr[k];
-        d.lp_ctl[9] += 1ull;
-        for (int k = 0; k < 3; ++k) d.lp_ctl[10 + k] += own[k];   // CTA 0 as an owner: steps, ns correcting, ns publishing
+        ctl[2] += (unsigned long long)psteps;
+        ctl[3] += (unsigned long long)(steps - ct_steps0);
+        ctl[4] += gd_gtime<TIMERS>() - g_begin;
+        for (int k = 0; k < 4; ++k) ctl[5 + k] += tr[k];
+        ctl[9] += 1ull;
+        for (int k = 0; k < 3; ++k) ctl[10 + k] += own[k];   // CTA 0 as an owner: steps, ns correcting, ns publishing
     }
 }
 
@@ -1052,14 +1065,15 @@ int gdk_loop_setup(gd_ctx *c)
     GD_CUDA(c, cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     GD_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     size_t avail = (size_t)max_smem;
-    if (gd_raise_smem_limit(c, k_block_loop<false>, max_smem, &avail) || gd_raise_smem_limit(c, k_block_loop<true>, max_smem, &avail))
+    if (gd_raise_smem_limit(c, k_block_loop<false, false>, max_smem, &avail) || gd_raise_smem_limit(c, k_block_loop<true, false>, max_smem, &avail) ||
+        gd_raise_smem_limit(c, k_block_loop<false, true>, max_smem, &avail) || gd_raise_smem_limit(c, k_block_loop<true, true>, max_smem, &avail))
         return -3;                                           // GD_ECUDA; text already in c->err
     int state = c->loop_state_opt ? 1 : 0;
     size_t bytes = gd_lsm_bytes((int)S, state);
     if (bytes > avail) { state = 0; bytes = gd_lsm_bytes((int)S, 0); }
     if (!coop || bytes > avail) return 0;
     int resident = 0;
-    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_block_loop<false>, GD_LP_THREADS, bytes));
+    GD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_block_loop<false, true>, GD_LP_THREADS, bytes));
     if (resident < 1) return 0;
     c->loop_grid = grid;
     c->loop_S = (int)S;
@@ -1092,7 +1106,9 @@ int gdk_loop(gd_ctx *c)
     la.ext = 0;
     la.ext_idx = nullptr;
     void *args[] = {(void *)&c->d, (void *)&la};
-    const void *fn = (c->eps2 < 2.3e-308) ? (const void *)k_block_loop<true> : (const void *)k_block_loop<false>;
+    const bool eps0 = c->eps2 < 2.3e-308, timers = GD_LP_PROFILE && c->loop_timers;
+    const void *fn = eps0 ? (timers ? (const void *)k_block_loop<true, true> : (const void *)k_block_loop<true, false>)
+                          : (timers ? (const void *)k_block_loop<false, true> : (const void *)k_block_loop<false, false>);
     cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)c->loop_grid), dim3(GD_LP_THREADS), args, c->loop_smem, c->stream);
     if (e != cudaSuccess) return gd_fail_cuda(c, e, "k_block_loop");
     c->launches += 1;

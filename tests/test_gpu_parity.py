@@ -440,6 +440,32 @@ def test_loop_tiny_systems_and_eps0(gd):
     h.close()
 
 
+def test_loop_timers_are_off_by_default_and_change_nothing(gd):
+    # the default instantiation of k_block_loop has no timers: step counts are kept, every ns stays 0 and nothing is
+    # binned; "loop_timers" switches to the instantiation with timers, which must take the very same steps
+    w = W.config(1, n=900)
+    plain = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    timed = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    timed.set_option("loop_timers", 1)
+    plain.step(150); timed.step(150)
+    lp, lt = plain.loop_profile(), timed.loop_profile()
+    assert lp["block_steps"] == lt["block_steps"] == 150 and lp["particle_steps"] == lt["particle_steps"]
+    assert all(v == 0 for k, v in lp.items() if k.startswith("ns")) and plain.loop_histogram() == []
+    assert lt["ns"] > 0 and lt["ns_force"] > 0
+    rows = timed.loop_histogram()
+    assert sum(r["block_steps"] for r in rows) == 150 and sum(r["particle_steps"] for r in rows) == lt["particle_steps"]
+    a, b = plain.state_host(), timed.state_host()
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+    timed.set_option("loop_timers", 0)          # back to the plain instantiation: the graph is rebuilt, the bins stop growing
+    timed.step(50); plain.step(50)
+    assert sum(r["block_steps"] for r in timed.loop_histogram()) == 150 and timed.loop_profile()["block_steps"] == 200
+    a, b = plain.state_host(), timed.state_host()
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+    plain.close(); timed.close()
+
+
 def test_loop_resumes_and_honours_max_steps(gd):
     w = W.config(1, n=700)
     h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
