@@ -256,7 +256,7 @@ def stage_bandwidth(gd, torch, W):
     s_nb = statistics.median(timed(h.next_block)[0] for _ in range(9))     # median of nine single calls
     rows["next_block"] = {"us": round(s_nb * 1e6, 2), "n_act": n_first, "algorithmic_bytes": 16.0 * w.n + 4.0 * n_first,
                           "gbs": (16.0 * w.n + 4.0 * n_first) / s_nb / 1e9, "frac_hbm": (16.0 * w.n + 4.0 * n_first) / s_nb / 1e9 / peak,
-                          "note": "per call, including the device-to-host copy of (t_next, n_act) and the stream synchronisation"}
+                          "note": "per call, including the stream synchronisation; the one-kernel form writes (t_next, n_act) into mapped pinned host words itself, so there is no separate device-to-host copy"}
     h.energy()                                         # a6 at this size (warm-up call, then one timed call)
     sec_en, _ = timed(h.energy)
     h.set_option("dt_level_min", 10)
@@ -402,7 +402,9 @@ def ncu_traffic(workload: str, kernel: str):
     """dram bytes per launch of `kernel` from the committed `ncu --set full` capture, if profiles/ncu_traffic.csv holds a
     row for this workload and kernel (columns: workload, kernel, dram_bytes, ..., profile, commit; the command that
     made it is in the profile file named there).  A capture is a property of the commit it was taken at, so the row
-    names it; no row -> None."""
+    names it, together with the kernel's source file and the first 16 hex digits of that file's SHA-256 at the capture:
+    `stale` says whether the file in this tree still has that digest (there is no .git on the GPU box to ask).
+    No row -> None."""
     try:
         lines = (ROOT / "profiles" / "ncu_traffic.csv").read_text().strip().splitlines()
     except OSError:
@@ -411,7 +413,14 @@ def ncu_traffic(workload: str, kernel: str):
     for ln in lines[1:]:
         row = dict(zip(head, ln.split(",")))
         if row.get("workload") == workload and row.get("kernel") == kernel:
-            return float(row["dram_bytes"]), {"profile": row.get("profile"), "commit": row.get("commit")}
+            src = {"profile": row.get("profile"), "commit": row.get("commit"), "stale": None}
+            if row.get("source") and row.get("source_sha16"):
+                try:
+                    import hashlib
+                    src["stale"] = hashlib.sha256((ROOT / row["source"]).read_bytes()).hexdigest()[:16] != row["source_sha16"]
+                except OSError:
+                    pass
+            return float(row["dram_bytes"]), src
     return None, None
 
 
@@ -524,6 +533,7 @@ def finish_ours(args, gd, W, torch, w, t_end, world, results, e2e_results, sec, 
         "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_NOMINAL_TFLOPS,
         "traffic": ncu_traffic(args.workload, KERNEL_NAMES[dom])[0],
         "traffic_source": ncu_traffic(args.workload, KERNEL_NAMES[dom])[1],
+        "traffic_stale": (ncu_traffic(args.workload, KERNEL_NAMES[dom])[1] or {}).get("stale"),
         "peak_source": "derived: 148 SM x 64 DFMA lanes/clk x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
                        "entry); register-only DFMA probe on this box: %.2f TFLOP/s" % (peak_probe / 1e12),
         "launches": int(d["launches"]), "avg_launch_us": 1e3 * d["ms"] / max(d["launches"], 1),

@@ -6,6 +6,7 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <cmath>
 
 static char g_init_err[512] = "";
 
@@ -463,6 +464,11 @@ extern "C" int gd_core_radius(gd_ctx *c, int k_neighbours, double *core_radius_h
     GD_CUDA(c, cudaStreamSynchronize(c->stream));
     *core_radius_host = out[3];
     if (density_centre_host) { density_centre_host[0] = out[0]; density_centre_host[1] = out[1]; density_centre_host[2] = out[2]; }
+    // a particle with K others on its own point has r_iK = 0 and an infinite (or 0/0) density: the weighted means are then NaN.  The values
+    // are handed back as computed, but not as a success.
+    if (!std::isfinite(out[5]) || !std::isfinite(out[3]) || !std::isfinite(out[4]))
+        return gd_fail(c, GD_EINVAL, "gd_core_radius: a particle has its k-th neighbour at distance 0 (coincident particles): "
+                                     "the density estimate is not finite");
     return GD_OK;
 }
 

@@ -209,15 +209,17 @@ int gdk_census(gd_ctx *c, unsigned long long *counts_dev)
 #define GD_KNN_MAXK 8
 #define GD_KNN_TILE 256
 
-__global__ void __launch_bounds__(GD_KNN_TILE) k_diag_knn(gd_dev d, int64_t n, int K, double *rho)
+template <int K>
+__global__ void __launch_bounds__(GD_KNN_TILE) k_diag_knn(gd_dev d, int64_t n, double *rho)
 {
+    static_assert(K >= 2 && K <= GD_KNN_MAXK, "k_diag_knn: 2 <= K <= GD_KNN_MAXK");
     __shared__ double2 s_xy[GD_KNN_TILE], s_zm[GD_KNN_TILE];
     const int64_t i = (int64_t)blockIdx.x * GD_KNN_TILE + threadIdx.x;
     const bool live = i < n;
     const double2 xy = live ? d.pxy[i] : make_double2(0.0, 0.0), zm = live ? d.pzm[i] : make_double2(0.0, 0.0);
-    double r2k[GD_KNN_MAXK], mk[GD_KNN_MAXK];
+    double r2k[K], mk[K];                                    // only the K nearest are kept: a source enters if closer than the K-th
 #pragma unroll
-    for (int k = 0; k < GD_KNN_MAXK; ++k) { r2k[k] = __longlong_as_double(0x7ff0000000000000LL); mk[k] = 0.0; }
+    for (int k = 0; k < K; ++k) { r2k[k] = __longlong_as_double(0x7ff0000000000000LL); mk[k] = 0.0; }
     for (int64_t j0 = 0; j0 < n; j0 += GD_KNN_TILE) {
         const int64_t j = j0 + threadIdx.x;
         __syncthreads();
@@ -228,11 +230,11 @@ __global__ void __launch_bounds__(GD_KNN_TILE) k_diag_knn(gd_dev d, int64_t n, i
             const double2 sxy = s_xy[t], szm = s_zm[t];
             const double dx = __dsub_rn(sxy.x, xy.x), dy = __dsub_rn(sxy.y, xy.y), dz = __dsub_rn(szm.x, zm.x);
             const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            if (r2 < r2k[GD_KNN_MAXK - 1] && j0 + t != i) {
+            if (r2 < r2k[K - 1] && j0 + t != i) {
                 // insert, keeping the list ascending; an equal distance goes behind the ones already there
                 double cr = r2, cm = szm.y;
 #pragma unroll
-                for (int k = 0; k < GD_KNN_MAXK; ++k) {
+                for (int k = 0; k < K; ++k) {
                     if (cr < r2k[k]) {
                         const double tr = r2k[k], tm = mk[k];
                         r2k[k] = cr; mk[k] = cm;
@@ -244,19 +246,16 @@ __global__ void __launch_bounds__(GD_KNN_TILE) k_diag_knn(gd_dev d, int64_t n, i
     }
     if (!live) return;
     // the K - 1 nearest masses, nearest first; the sphere through the K-th
-    double mass = 0.0, rK2 = r2k[0];
+    double mass = 0.0;
 #pragma unroll
-    for (int k = 0; k < GD_KNN_MAXK; ++k) {
-        if (k < K - 1) mass = __dadd_rn(mass, mk[k]);
-        if (k == K - 1) rK2 = r2k[k];
-    }
-    const double r = __dsqrt_rn(rK2);
+    for (int k = 0; k < K - 1; ++k) mass = __dadd_rn(mass, mk[k]);
+    const double r = __dsqrt_rn(r2k[K - 1]);
     const double c43 = 4.0 * 3.141592653589793 / 3.0;
     rho[i] = __ddiv_rn(mass, __dmul_rn(__dmul_rn(__dmul_rn(c43, r), r), r));
 }
 
 // x_d and r_c from rho (fixed order: a contiguous slice per thread in index order, then a binary tree) -> out[0..2] = x_d,
-// out[3] = r_c, out[4] = sum rho, out[5] = largest rho_i
+// out[3] = r_c, out[4] = sum rho, out[5] = largest rho_i (+inf when a particle has K others on its own point: gd_core_radius reports that)
 __global__ void __launch_bounds__(1024) k_diag_core(gd_dev d, int64_t n, const double *rho, double *out)
 {
     __shared__ double s[4][1024];
@@ -304,7 +303,13 @@ __global__ void __launch_bounds__(1024) k_diag_core(gd_dev d, int64_t n, const d
 int gdk_core_radius(gd_ctx *c, int K, double *rho_dev, double *out_dev)
 {
     double *rho = rho_dev ? rho_dev : c->d.phi;
-    k_diag_knn<<<(unsigned)((c->n + GD_KNN_TILE - 1) / GD_KNN_TILE), GD_KNN_TILE, 0, c->stream>>>(c->d, c->n, K, rho);
+    const unsigned blocks = (unsigned)((c->n + GD_KNN_TILE - 1) / GD_KNN_TILE);
+    switch (K) {
+#define GD_KNN_CASE(k) case k: k_diag_knn<k><<<blocks, GD_KNN_TILE, 0, c->stream>>>(c->d, c->n, rho); break;
+        GD_KNN_CASE(2) GD_KNN_CASE(3) GD_KNN_CASE(4) GD_KNN_CASE(5) GD_KNN_CASE(6) GD_KNN_CASE(7) GD_KNN_CASE(8)
+#undef GD_KNN_CASE
+        default: return -1;                                  // GD_EINVAL: gd_core_radius checks the range before
+    }
     GD_LAUNCH_CHECK(c, "k_diag_knn");
     k_diag_core<<<1, 1024, 0, c->stream>>>(c->d, c->n, rho, out_dev);
     GD_LAUNCH_CHECK(c, "k_diag_core");

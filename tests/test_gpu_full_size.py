@@ -95,6 +95,44 @@ def test_full_size_all_active_sampled_sinks(gd, cfg):
     h.close()
 
 
+def test_c4_all_active_steps_inside_the_block_loop_match_oracle(gd):
+    # The path that does most of C4's arithmetic: k_block_loop with tens of thousands of sinks per step (lanes over
+    # sinks, 148 partial rows per sink, owners fold and correct).  A shared step (dt_level_min = dt_level_max) makes every
+    # block step all-active at N = 262144; gd_run_until takes them inside the loop.  Sampled sinks one by one: a, jerk of
+    # the second step against the oracle's sums over the state the device held before it (predicted by the oracle, which
+    # the predictor parity test shows bit-identical), and the corrected x, v, t, dt against the oracle's corrector.
+    w = W.config(4)
+    lvl = 12
+    dt = 2.0 ** -lvl
+    h = gd.Hermite(w.m, w.x, w.v, w.eps, w.eta)
+    h.set_option("dt_level_min", lvl)
+    h.set_option("dt_level_max", lvl)
+    steps, psteps = h.run_until(dt)
+    assert (steps, psteps) == (1, w.n) and h.loop_profile()["block_steps"] == 1
+    s1 = h.state_host()
+    assert np.all(s1["t"] == dt) and np.all(s1["dt"] == dt)
+    steps, psteps = h.run_until(2 * dt)
+    assert (steps, psteps) == (1, w.n) and h.loop_profile()["block_steps"] == 2 and h.loop_profile()["particle_steps"] == 2 * w.n
+    s2 = h.state_host()
+    h.close()
+    idx = W.active_indices(w.n, 509, seed=904)
+    xp, vp = oracle.predict(2 * dt, s1["x"], s1["v"], s1["a"], s1["j"], s1["t"])
+    a_ref, j_ref = oracle.pairsum(w.m, xp, vp, w.eps, idx=idx)
+    ea, ej = relnorm(s2["a"][idx], a_ref), relnorm(s2["j"][idx], j_ref)
+    assert ea.max() <= TOL and ej.max() <= TOL, (ea.max(), ej.max())
+    ref = oracle.correct(idx, 2 * dt, w.eta, s1["x"], s1["v"], s1["a"], s1["j"], s1["t"], s1["dt"], xp, vp, a_ref, j_ref,
+                         dt_min=dt, dt_max=dt)
+    for k, r in zip(("x", "v", "t", "dt"), (ref[0], ref[1], ref[4], ref[5])):
+        if k in ("t", "dt"):
+            assert np.array_equal(s2[k][idx], r[idx]), k
+        else:
+            assert np.abs(s2[k][idx] - r[idx]).max() <= 1e-12 * max(1.0, np.abs(r[idx]).max()), k
+    # the whole output: finite, momentum of the accelerations vanishes to rounding
+    assert np.isfinite(s2["a"]).all() and np.isfinite(s2["j"]).all()
+    tot = (w.m[:, None] * s2["a"]).sum(axis=0)
+    assert np.abs(tot).max() <= 1e-12 * (w.m * np.linalg.norm(s2["a"], axis=1)).sum()
+
+
 # ------------------------------------------------------------------ first 100 block steps at full size (stored)
 def read_schedule(cfg):
     steps, kv, samples = [], {}, []

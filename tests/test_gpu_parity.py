@@ -520,10 +520,17 @@ def test_lagrange_radii_match_oracle(gd, cfg, n):
     assert abs(mtot - w.m.sum()) <= 1e-14 * w.m.sum() and np.abs(c - c_ref).max() < 1e-14
     # (C5's central particle sits on the centre of mass: its distance is the rounding noise of the centre)
     assert np.all(np.abs(r - r_ref) <= 1e-12 * r_ref + 1e-14), (r, r_ref)
+    # and directly against the definition of P:306 written out (plain float cumulative mass, no fixed point): on these
+    # inputs it names the same particle per fraction as the fixed-point count, so the device gives that particle's radius
+    r_plain, c_plain, who = lagrange.lagrange_radii_plain(w.m, w.x, fr)
+    assert np.array_equal(r_plain, r_ref), "the fixed-point and the plain cumulative mass name different particles here"
+    assert np.abs(c - c_plain).max() < 1e-14 and np.all(np.abs(r - r_plain) <= 1e-12 * r_plain + 1e-14), (r, r_plain)
+    assert np.allclose(np.linalg.norm(w.x[who] - c, axis=1), r, rtol=1e-12, atol=1e-14)
     # about a given centre the centre drops out of the comparison: identical bits
     r2, c2, _ = h.lagrange_radii(fr, center=[0.05, -0.1, 0.2])
     r2_ref, _ = lagrange.lagrange_radii(w.m, w.x, fr, centre=[0.05, -0.1, 0.2])
     assert np.array_equal(r2, r2_ref) and np.array_equal(c2, [0.05, -0.1, 0.2])
+    assert np.array_equal(r2, lagrange.lagrange_radii_plain(w.m, w.x, fr, centre=[0.05, -0.1, 0.2])[0])
     h.close()
 
 
@@ -673,6 +680,22 @@ def test_core_radius_matches_oracle(gd, cfg, n, k):
     for bad in (1, 9):
         with pytest.raises(gd.GravidyError):
             h.core_radius(bad)
+    h.close()
+
+
+def test_core_radius_reports_coincident_particles(gd):
+    # a particle with K others on its own point: r_iK = 0, the density estimate is infinite and the weighted means NaN --
+    # an error, not GD_OK
+    w = W.config(1, n=300)
+    x = w.x.copy()
+    x[10:16] = x[10]                       # six coincident particles: each has five neighbours at distance 0
+    h = gd.Hermite(w.m, x, w.v, 1e-2, w.eta)
+    for k in (8, 6):                       # the 6th neighbour is somewhere else: fine
+        rc, _ = h.core_radius(k)
+        assert np.isfinite(rc) and rc > 0
+    for k in (5, 2):
+        with pytest.raises(gd.GravidyError, match="coincident"):
+            h.core_radius(k)
     h.close()
 
 
